@@ -1,0 +1,184 @@
+"""Python binding of libbang.so (include/bang.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; PyTorch is used for device memory and streams.
+There is no CPU fallback: if the shared library is missing or no CUDA device is present, calls fail loudly.
+The function names mirror the C ABI: create / set_data / model_maps / model_fine / loglike (+ *_host).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbang.so")
+
+BULGE, DISC1, DISC2, HALO = 1, 2, 4, 8
+HALO_HERNQUIST, HALO_NFW = 0, 1
+FP32, FP64 = 0, 1
+NTHETA = 17
+OK, EINVAL, ENOMEM, ECUDA, ENODATA = 0, -1, -2, -3, -4
+
+EXPORTS = ["bang_create", "bang_set_data", "bang_model_maps", "bang_model_fine", "bang_loglike", "bang_loglike_host",
+           "bang_model_maps_host", "bang_get_geometry", "bang_launch_count", "bang_destroy", "bang_strerror",
+           "bang_last_error"]
+
+
+class Grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("pix_arcsec", C.c_double), ("supersample", C.c_int),
+                ("dist_mpc", C.c_double)]
+
+
+class Psf(C.Structure):
+    _fields_ = [("sigma_pix", C.c_double), ("trunc_nsigma", C.c_double)]
+
+
+class Model(C.Structure):
+    _fields_ = [("components", C.c_uint), ("bulge_profile", C.c_int), ("halo_profile", C.c_int),
+                ("jeans_nodes", C.c_int), ("precision", C.c_int)]
+
+
+class BangError(RuntimeError):
+    def __init__(self, code, detail=""):
+        self.code = code
+        super().__init__(f"libbang error {code}: {detail}")
+
+
+_lib = None
+
+
+def lib():
+    """Load libbang.so (built in-tree by paper_2205_06819_b200.build).  Raises if it is not there."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not found: run `python -m paper_2205_06819_b200.build` "
+                                    "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, ip, dp = C.c_void_p, C.c_int, C.c_double
+        L.bang_create.argtypes = [C.POINTER(vp), C.POINTER(Grid), C.POINTER(Psf), C.POINTER(Model), ip, vp]
+        L.bang_create.restype = ip
+        L.bang_set_data.argtypes = [vp, vp, vp, vp]
+        L.bang_set_data.restype = ip
+        for name in ("bang_model_maps", "bang_model_fine", "bang_loglike", "bang_loglike_host", "bang_model_maps_host"):
+            f = getattr(L, name)
+            f.argtypes, f.restype = [vp, vp, ip, vp], ip
+        L.bang_get_geometry.argtypes = [vp, C.POINTER(ip), C.POINTER(ip), C.POINTER(ip)]
+        L.bang_get_geometry.restype = ip
+        L.bang_launch_count.argtypes, L.bang_launch_count.restype = [vp], C.c_longlong
+        L.bang_destroy.argtypes, L.bang_destroy.restype = [vp], None
+        L.bang_strerror.argtypes, L.bang_strerror.restype = [ip], C.c_char_p
+        L.bang_last_error.argtypes, L.bang_last_error.restype = [vp], C.c_char_p
+        _lib = L
+    return _lib
+
+
+class Context:
+    """One bang_ctx: a grid, a PSF, a model variant and a precision, bound to a CUDA device and stream."""
+
+    def __init__(self, cfg: dict, precision: str | None = None, device: int = 0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("bang.Context needs a CUDA device (there is no CPU fallback)")
+        self._torch = torch
+        self.cfg = dict(cfg)
+        prec = precision or cfg.get("precision", "fp32")
+        self.precision = prec
+        self.dtype = torch.float64 if prec == "fp64" else torch.float32
+        self.np_dtype = np.float64 if prec == "fp64" else np.float32
+        self.device = torch.device("cuda", device)
+        self.nx, self.ny, self.s = int(cfg["nx"]), int(cfg["ny"]), int(cfg["supersample"])
+        g = Grid(self.nx, self.ny, float(cfg["pix_arcsec"]), self.s, float(cfg["dist_mpc"]))
+        p = Psf(float(cfg["sigma_pix"]), float(cfg.get("trunc_nsigma", 3.0)))
+        m = Model(int(cfg["components"]), 0, int(cfg.get("halo_profile", 0)), int(cfg["jeans_nodes"]),
+                  FP64 if prec == "fp64" else FP32)
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = C.c_void_p()
+        rc = lib().bang_create(C.byref(h), C.byref(g), C.byref(p), C.byref(m), device,
+                               C.c_void_p(self._stream.cuda_stream))
+        if rc != OK:
+            raise BangError(rc, lib().bang_strerror(rc).decode())
+        self._h = h
+        rk, nfx, nfy = C.c_int(), C.c_int(), C.c_int()
+        lib().bang_get_geometry(self._h, C.byref(rk), C.byref(nfx), C.byref(nfy))
+        self.r_k, self.nfx, self.nfy = rk.value, nfx.value, nfy.value
+
+    # -- helpers
+    def _check(self, rc):
+        if rc != OK:
+            raise BangError(rc, lib().bang_last_error(self._h).decode() or lib().bang_strerror(rc).decode())
+
+    def _theta(self, theta):
+        torch = self._torch
+        t = torch.as_tensor(theta, dtype=torch.float64, device=self.device).reshape(-1, NTHETA).contiguous()
+        return t
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().bang_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def launches(self) -> int:
+        return int(lib().bang_launch_count(self._h))
+
+    # -- the ABI calls
+    def set_data(self, data, err, mask):
+        torch = self._torch
+        d = torch.as_tensor(data, dtype=torch.float64, device=self.device).contiguous()
+        e = torch.as_tensor(err, dtype=torch.float64, device=self.device).contiguous()
+        m = torch.as_tensor(np.asarray(mask, dtype=np.uint8) if not torch.is_tensor(mask) else mask,
+                            dtype=torch.uint8, device=self.device).contiguous()
+        assert d.shape == (4, self.ny, self.nx) and e.shape == d.shape and m.shape == d.shape
+        self._check(lib().bang_set_data(self._h, d.data_ptr(), e.data_ptr(), m.data_ptr()))
+
+    def model_maps(self, theta, out=None):
+        """theta [B][17] (tensor on the device, or array-like) -> maps [B][4][ny][nx] device tensor (async)."""
+        torch = self._torch
+        t = self._theta(theta)
+        B = t.shape[0]
+        if out is None:
+            out = torch.empty((B, 4, self.ny, self.nx), dtype=self.dtype, device=self.device)
+        self._check(lib().bang_model_maps(self._h, t.data_ptr(), B, out.data_ptr()))
+        return out
+
+    def model_fine(self, theta):
+        torch = self._torch
+        t = self._theta(theta)
+        B = t.shape[0]
+        out = torch.empty((B, 4, self.nfy, self.nfx), dtype=self.dtype, device=self.device)
+        self._check(lib().bang_model_fine(self._h, t.data_ptr(), B, out.data_ptr()))
+        return out
+
+    def loglike(self, theta, out=None):
+        """theta [B][17] device tensor -> logL [B] float64 device tensor (async on the context's stream)."""
+        torch = self._torch
+        t = self._theta(theta)
+        B = t.shape[0]
+        if out is None:
+            out = torch.empty((B,), dtype=torch.float64, device=self.device)
+        self._check(lib().bang_loglike(self._h, t.data_ptr(), B, out.data_ptr()))
+        return out
+
+    def loglike_host(self, theta: np.ndarray, out: np.ndarray | None = None) -> np.ndarray:
+        """HOST numpy theta [B][17] -> HOST numpy logL [B]; copies and synchronisation inside the call."""
+        t = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, NTHETA)
+        B = t.shape[0]
+        if out is None:
+            out = np.empty(B, dtype=np.float64)
+        self._check(lib().bang_loglike_host(self._h, t.ctypes.data, B, out.ctypes.data))
+        return out
+
+    def model_maps_host(self, theta: np.ndarray) -> np.ndarray:
+        t = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, NTHETA)
+        B = t.shape[0]
+        out = np.empty((B, 4, self.ny, self.nx), dtype=self.np_dtype)
+        self._check(lib().bang_model_maps_host(self._h, t.ctypes.data, B, out.ctypes.data))
+        return out

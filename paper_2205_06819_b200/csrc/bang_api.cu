@@ -1,0 +1,508 @@
+// bang_api.cu -- the C ABI of include/bang.h: context, one-off table kernels, data preparation, launches.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/bang.h"
+#include "bang_host.h"
+
+using namespace bang;
+
+struct bang_ctx {
+    bang_grid grid{};
+    bang_psf psf{};
+    bang_model model{};
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int n_sm = 0;
+    GridC g{};
+    FitC fit{};
+    int rk = 0, nacc = 0, P = 0, nxp = 0, nfb = 0, threads = 0;
+    std::vector<double> W;                 // composite taps, nacc * s
+    void* btab = nullptr; int btab_first = 0, btab_cells = 0;
+    void* Ftab = nullptr; int Ftab_first = 0, Ftab_cells = 0;
+    double2* data = nullptr; double C0 = 0.0; bool has_data = false;
+    double* scal = nullptr;                // device scratch: {C0, bad-pixel count}
+    // staging for the *_host calls
+    double* h_theta = nullptr; double* d_theta = nullptr; void* h_out = nullptr; void* d_out = nullptr;
+    size_t cap_theta = 0, cap_out = 0;
+    long long launches = 0;
+    int force_ctas = 0;
+    char err[512] = {0};
+};
+
+namespace {
+
+int fail(bang_ctx* c, int code, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+#define CU(call)                                                                                              \
+    do {                                                                                                      \
+        cudaError_t e_ = (call);                                                                              \
+        if (e_ != cudaSuccess)                                                                                \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? BANG_ENOMEM : BANG_ECUDA, "%s: %s", #call,    \
+                        cudaGetErrorString(e_));                                                              \
+    } while (0)
+
+// Gauss-Legendre nodes and weights on (-1,1): Newton iteration on P_n (Abramowitz & Stegun 25.4.29), long double
+void gauss_legendre(int n, double* x, double* w) {
+    for (int i = 0; i < (n + 1) / 2; ++i) {
+        long double z = cosl(3.14159265358979323846264338328L * (i + 0.75L) / (n + 0.5L)), pp = 1;
+        for (int it = 0; it < 100; ++it) {
+            long double p0 = 1, p1 = z;
+            for (int j = 2; j <= n; ++j) {
+                long double p2 = ((2 * j - 1) * z * p1 - (j - 1) * p0) / j;
+                p0 = p1; p1 = p2;
+            }
+            pp = n * (z * p1 - p0) / (z * z - 1);
+            long double dz = p1 / pp;
+            z -= dz;
+            if (fabsl(dz) < 1e-19L) break;
+        }
+        {   // derivative at the converged root
+            long double p0 = 1, p1 = z;
+            for (int j = 2; j <= n; ++j) {
+                long double p2 = ((2 * j - 1) * z * p1 - (j - 1) * p0) / j;
+                p0 = p1; p1 = p2;
+            }
+            pp = n * (z * p1 - p0) / (z * z - 1);
+        }
+        x[i] = (double)-z; x[n - 1 - i] = (double)z;
+        w[i] = w[n - 1 - i] = (double)(2 / ((1 - z * z) * pp * pp));
+    }
+}
+
+// Chebyshev nodes t_k = cos(pi (k + 1/2)/(D+1)) and the inverse of the Vandermonde matrix V[k][d] = t_k^d
+void make_fit(int D, FitC& fit) {
+    const int n = D + 1;
+    long double A[8][16];
+    for (int k = 0; k < n; ++k) {
+        long double t = cosl(3.14159265358979323846264338328L * (k + 0.5L) / n), p = 1;
+        fit.tnode[k] = (double)t;
+        for (int d = 0; d < n; ++d) { A[k][d] = p; p *= t; }
+        for (int d = 0; d < n; ++d) A[k][n + d] = (d == k) ? 1 : 0;
+    }
+    for (int c = 0; c < n; ++c) {                      // Gauss-Jordan with partial pivoting
+        int piv = c;
+        for (int r = c + 1; r < n; ++r) if (fabsl(A[r][c]) > fabsl(A[piv][c])) piv = r;
+        for (int j = 0; j < 2 * n; ++j) { long double t = A[c][j]; A[c][j] = A[piv][j]; A[piv][j] = t; }
+        long double inv = 1 / A[c][c];
+        for (int j = 0; j < 2 * n; ++j) A[c][j] *= inv;
+        for (int r = 0; r < n; ++r)
+            if (r != c) {
+                long double f = A[r][c];
+                for (int j = 0; j < 2 * n; ++j) A[r][j] -= f * A[c][j];
+            }
+    }
+    for (int d = 0; d < n; ++d)
+        for (int k = 0; k < n; ++k) fit.vinv[d * n + k] = (double)A[d][n + k];
+}
+
+// ---- one-off kernels: the scale-free tables (K0) ---------------------------------------------
+// which = 0: Hernquist SigmaTilde(s) and the N_J-node Jeans integral J(s), at u = s^2;  which = 1: Freeman F(y), u = y^2
+template <typename T>
+__global__ void k_univ_nodes(int which, int first, int n_cells, FitC fit, int NJ, const double* __restrict__ glx,
+                             const double* __restrict__ glw, double* __restrict__ vals) {
+    constexpr int NC = TabCfg<T>::D + 1;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_cells * NC) return;
+    const int cell = i / NC, k = i - cell * NC;
+    double lo, width;
+    tab_interval<T>(first + cell, lo, width);
+    const double x = sqrt(lo + 0.5 * width * (fit.tnode[k] + 1.0));
+    if (which == 0) {
+        vals[(cell * 2 + 0) * NC + k] = sigma_tilde(x);
+        vals[(cell * 2 + 1) * NC + k] = jeans_J(x, NJ, glx, glw);
+    } else {
+        vals[cell * NC + k] = freeman_F(x);
+    }
+}
+template <typename T>
+__global__ void k_univ_fit(int n_rows, FitC fit, const double* __restrict__ vals, T* __restrict__ coef) {
+    constexpr int NC = TabCfg<T>::D + 1;
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_rows) return;
+    for (int d = 0; d < NC; ++d) {
+        double a = 0.0;
+        for (int k = 0; k < NC; ++k) a = fma(fit.vinv[d * NC + k], vals[r * NC + k], a);
+        coef[r * NC + d] = (T)a;
+    }
+}
+
+// data preparation: {d, 1/e} per used pixel ({0,0} where masked or padded), C0 = sum -1/2 ln(2 pi e^2), and the number
+// of used pixels with err <= 0 or a non-finite value.  One block, deterministic reduction order.
+__global__ void k_prep_data(int nx, int ny, int nxp, const double* __restrict__ data, const double* __restrict__ err,
+                            const unsigned char* __restrict__ mask, double2* __restrict__ out, double* __restrict__ scal) {
+    __shared__ double sh[2][32];
+    double c0 = 0.0, bad = 0.0;
+    const int total = ny * 4 * nxp;
+    for (int i = threadIdx.x; i < total; i += blockDim.x) {
+        const int px = i % nxp, q = (i / nxp) % 4, py = i / (4 * nxp);
+        double2 v = make_double2(0.0, 0.0);
+        if (px < nx) {
+            const size_t src = ((size_t)q * ny + py) * nx + px;
+            if (mask[src]) {
+                const double d = data[src], e = err[src];
+                if (!(e > 0.0) || !isfinite(e) || !isfinite(d)) bad += 1.0;
+                else {
+                    v = make_double2(d, 1.0 / e);
+                    c0 += -0.5 * log(2.0 * kPi * e * e);
+                }
+            }
+        }
+        out[i] = v;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        c0 += __shfl_xor_sync(0xffffffffu, c0, o);
+        bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) { sh[0][threadIdx.x >> 5] = c0; sh[1][threadIdx.x >> 5] = bad; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int w = 0; w < (int)(blockDim.x + 31) / 32; ++w) { a += sh[0][w]; b += sh[1][w]; }
+        scal[0] = a; scal[1] = b;
+    }
+}
+
+template <typename T>
+int build_universal(bang_ctx* ctx, const double* glx_dev, const double* glw_dev) {
+    constexpr int NC = TabCfg<T>::D + 1;
+    ctx->btab_first = tab_first_cell<T>(kBulgeOctLo);
+    ctx->btab_cells = (kBulgeOctHi - kBulgeOctLo) << TabCfg<T>::M;
+    ctx->Ftab_first = tab_first_cell<T>(kFOctLo);
+    ctx->Ftab_cells = (kFOctHi - kFOctLo) << TabCfg<T>::M;
+    double* vals = nullptr;
+    const size_t nb = (size_t)ctx->btab_cells * 2 * NC, nf = (size_t)ctx->Ftab_cells * NC;
+    CU(cudaMalloc(&vals, (nb + nf) * sizeof(double)));
+    CU(cudaMalloc(&ctx->btab, nb * sizeof(T)));
+    CU(cudaMalloc(&ctx->Ftab, nf * sizeof(T)));
+    const int th = 128;
+    k_univ_nodes<T><<<(ctx->btab_cells * NC + th - 1) / th, th, 0, ctx->stream>>>(0, ctx->btab_first, ctx->btab_cells, ctx->fit,
+                                                                                ctx->model.jeans_nodes, glx_dev, glw_dev, vals);
+    k_univ_nodes<T><<<(ctx->Ftab_cells * NC + th - 1) / th, th, 0, ctx->stream>>>(1, ctx->Ftab_first, ctx->Ftab_cells, ctx->fit, 0,
+                                                                                nullptr, nullptr, vals + nb);
+    k_univ_fit<T><<<(ctx->btab_cells * 2 + th - 1) / th, th, 0, ctx->stream>>>(ctx->btab_cells * 2, ctx->fit, vals,
+                                                                             static_cast<T*>(ctx->btab));
+    k_univ_fit<T><<<(ctx->Ftab_cells + th - 1) / th, th, 0, ctx->stream>>>(ctx->Ftab_cells, ctx->fit, vals + nb,
+                                                                         static_cast<T*>(ctx->Ftab));
+    ctx->launches += 4;
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(ctx->stream));
+    cudaFree(vals);
+    return BANG_OK;
+}
+
+cudaError_t dispatch_fused(const bang_ctx* c, const FusedLaunch& L, FusedInfo* info, bool query) {
+    const bool f64 = c->model.precision == BANG_FP64;
+    switch (c->g.s) {
+        case 1: return f64 ? launch_fused_double_1(L, info, query) : launch_fused_float_1(L, info, query);
+        case 2: return f64 ? launch_fused_double_2(L, info, query) : launch_fused_float_2(L, info, query);
+        case 3: return f64 ? launch_fused_double_3(L, info, query) : launch_fused_float_3(L, info, query);
+        case 4: return f64 ? launch_fused_double_4(L, info, query) : launch_fused_float_4(L, info, query);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+FusedLaunch make_launch(const bang_ctx* c, const double* theta, int B, int mode, void* maps, double* logL) {
+    FusedLaunch L{};
+    L.g = c->g; L.fit = c->fit;
+    L.btab = c->btab; L.btab_first = c->btab_first; L.btab_cells = c->btab_cells;
+    L.Ftab = c->Ftab; L.Ftab_first = c->Ftab_first; L.Ftab_cells = c->Ftab_cells;
+    L.W = c->W.data(); L.nacc = c->nacc;
+    L.theta = theta; L.B = B; L.P = c->P; L.nxp = c->nxp; L.nfb = c->nfb; L.mode = mode;
+    L.maps = maps; L.data = c->data; L.C0 = c->C0; L.logL = logL;
+    L.threads = c->threads; L.ctas = c->force_ctas; L.n_sm = c->n_sm; L.stream = c->stream;
+    return L;
+}
+
+int ensure_staging(bang_ctx* ctx, int B, size_t out_bytes) {
+    const size_t tb = (size_t)B * kNTheta * sizeof(double);
+    if (tb > ctx->cap_theta) {
+        if (ctx->h_theta) cudaFreeHost(ctx->h_theta);
+        if (ctx->d_theta) cudaFree(ctx->d_theta);
+        ctx->h_theta = nullptr; ctx->d_theta = nullptr; ctx->cap_theta = 0;
+        CU(cudaMallocHost(&ctx->h_theta, tb));
+        CU(cudaMalloc(&ctx->d_theta, tb));
+        ctx->cap_theta = tb;
+    }
+    if (out_bytes > ctx->cap_out) {
+        if (ctx->h_out) cudaFreeHost(ctx->h_out);
+        if (ctx->d_out) cudaFree(ctx->d_out);
+        ctx->h_out = nullptr; ctx->d_out = nullptr; ctx->cap_out = 0;
+        CU(cudaMallocHost(&ctx->h_out, out_bytes));
+        CU(cudaMalloc(&ctx->d_out, out_bytes));
+        ctx->cap_out = out_bytes;
+    }
+    return BANG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* bang_strerror(int code) {
+    switch (code) {
+        case BANG_OK: return "success";
+        case BANG_EINVAL: return "invalid argument or unsupported configuration";
+        case BANG_ENOMEM: return "out of memory";
+        case BANG_ECUDA: return "CUDA error";
+        case BANG_ENODATA: return "no data loaded (call bang_set_data first)";
+        default: return "unknown error";
+    }
+}
+
+const char* bang_last_error(const bang_ctx* ctx) { return ctx ? ctx->err : ""; }
+
+long long bang_launch_count(const bang_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int bang_get_geometry(const bang_ctx* ctx, int* r_k, int* nfx, int* nfy) {
+    if (!ctx) return BANG_EINVAL;
+    if (r_k) *r_k = ctx->rk;
+    if (nfx) *nfx = ctx->g.nfx;
+    if (nfy) *nfy = ctx->g.nfy;
+    return BANG_OK;
+}
+
+void bang_destroy(bang_ctx* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->btab); cudaFree(ctx->Ftab); cudaFree(ctx->data); cudaFree(ctx->scal);
+    cudaFree(ctx->d_theta); cudaFree(ctx->d_out);
+    if (ctx->h_theta) cudaFreeHost(ctx->h_theta);
+    if (ctx->h_out) cudaFreeHost(ctx->h_out);
+    delete ctx;
+}
+
+int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, const bang_model* model, int device,
+                void* cuda_stream) {
+    if (!out) return BANG_EINVAL;
+    *out = nullptr;
+    if (!grid || !psf || !model) return BANG_EINVAL;
+    if (grid->nx < 1 || grid->ny < 1 || grid->supersample < 1 || grid->supersample > 4 || !(grid->pix_arcsec > 0) ||
+        !(grid->dist_mpc > 0) || !std::isfinite(grid->pix_arcsec) || !std::isfinite(grid->dist_mpc))
+        return BANG_EINVAL;
+    if (!(psf->sigma_pix >= 0) || !(psf->trunc_nsigma >= 0) || !std::isfinite(psf->sigma_pix) || !std::isfinite(psf->trunc_nsigma))
+        return BANG_EINVAL;
+    if (!(model->components & (BANG_BULGE | BANG_DISC1 | BANG_DISC2)) || (model->components & ~15u)) return BANG_EINVAL;
+    if (model->bulge_profile != BANG_BULGE_HERNQUIST) return BANG_EINVAL;
+    if (model->halo_profile != BANG_HALO_HERNQUIST && model->halo_profile != BANG_HALO_NFW) return BANG_EINVAL;
+    if (model->jeans_nodes < 1 || model->jeans_nodes > 4096) return BANG_EINVAL;
+    if (model->precision != BANG_FP32 && model->precision != BANG_FP64) return BANG_EINVAL;
+
+    const int s = grid->supersample;
+    const int rk = (int)std::ceil(psf->trunc_nsigma * psf->sigma_pix * s - 1e-9);
+    const int nacc = round_nacc((2 * rk + s + s - 1) / s);
+    if (nacc < 0) return BANG_EINVAL;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return BANG_ECUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return BANG_ECUDA;
+
+    bang_ctx* ctx = new (std::nothrow) bang_ctx;
+    if (!ctx) return BANG_ENOMEM;
+    ctx->grid = *grid; ctx->psf = *psf; ctx->model = *model; ctx->device = device;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete ctx; return BANG_ECUDA; }
+    ctx->n_sm = prop.multiProcessorCount;
+
+    const bool f64 = model->precision == BANG_FP64;
+    ctx->rk = rk; ctx->nacc = nacc;
+    GridC& g = ctx->g;
+    g.nx = grid->nx; g.ny = grid->ny; g.s = s; g.rk = rk;
+    g.nfx = grid->nx * s + 2 * rk; g.nfy = grid->ny * s + 2 * rk;
+    g.jsx = rk - 0.5 + 0.5 * grid->nx * s; g.jsy = rk - 0.5 + 0.5 * grid->ny * s;
+    g.spx = s / grid->pix_arcsec;
+    g.h = grid->pix_arcsec * grid->dist_mpc * kKpcPerArcsecPerMpc / s;
+    g.comps = model->components; g.halo_profile = model->halo_profile;
+
+    // eq. 21 on the fine grid, separable (reading F): g[m] = exp(-m^2/(2 sigma_f^2)), normalised;
+    // composed with the s-cell box of the rebin: W[t] = (1/s) sum_{b<s} g[t - b], t = 0 .. 2 r_k + s - 1.
+    {
+        std::vector<long double> gk(2 * rk + 1);
+        const long double sf = (long double)psf->sigma_pix * s;
+        long double sum = 0;
+        for (int m = -rk; m <= rk; ++m) {
+            gk[m + rk] = sf > 0 ? expl(-0.5L * m * m / (sf * sf)) : (m == 0 ? 1.0L : 0.0L);
+            sum += gk[m + rk];
+        }
+        ctx->W.assign((size_t)nacc * s, 0.0);
+        for (int t = 0; t < 2 * rk + s; ++t) {
+            long double a = 0;
+            for (int b = 0; b < s; ++b) {
+                const int m = t - b;
+                if (m >= 0 && m <= 2 * rk) a += gk[m];
+            }
+            ctx->W[t] = (double)(a / sum / s);
+        }
+    }
+
+    // launch shape: P data pixels per thread in the PSF phase, one thread per (observable, pixel group)
+    const char* envP = getenv("BANG_P");
+    int P = f64 ? 2 : (grid->nx >= 96 ? 4 : 2);
+    if (envP && !f64 && (atoi(envP) == 2 || atoi(envP) == 4)) P = atoi(envP);
+    ctx->P = P;
+    ctx->nxp = (grid->nx + P - 1) / P * P;
+    const int items = 4 * ctx->nxp / P;
+    ctx->threads = std::max(128, (items + 31) / 32 * 32);
+    const char* envT = getenv("BANG_THREADS");
+    if (envT && atoi(envT) >= ctx->threads && atoi(envT) <= 512) ctx->threads = atoi(envT) / 32 * 32;
+    const char* envC = getenv("BANG_CTAS");
+    if (envC && atoi(envC) > 0) ctx->force_ctas = atoi(envC);
+    ctx->nfb = ((ctx->nxp - 1 + nacc) * s + 3) / 4 * 4 + 4;
+    if (ctx->threads > 512) { delete ctx; return BANG_EINVAL; }      // row too wide for one CTA
+    make_fit(f64 ? TabCfg<double>::D : TabCfg<float>::D, ctx->fit);
+
+    // N_J-node Gauss-Legendre rule (reading B), then the scale-free tables on the device
+    std::vector<double> gl(2 * (size_t)model->jeans_nodes);
+    gauss_legendre(model->jeans_nodes, gl.data(), gl.data() + model->jeans_nodes);
+    double* gl_dev = nullptr;
+    int rc = BANG_OK;
+    do {
+        if (cudaMalloc(&gl_dev, gl.size() * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
+        if (cudaMemcpyAsync(gl_dev, gl.data(), gl.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess) {
+            rc = BANG_ECUDA; break;
+        }
+        rc = f64 ? build_universal<double>(ctx, gl_dev, gl_dev + model->jeans_nodes)
+                 : build_universal<float>(ctx, gl_dev, gl_dev + model->jeans_nodes);
+        if (rc != BANG_OK) break;
+        if (cudaMalloc(&ctx->scal, 2 * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
+        // does the fused kernel fit (shared memory, registers)?
+        FusedLaunch L = make_launch(ctx, nullptr, 1, 0, nullptr, nullptr);
+        FusedInfo info{};
+        cudaError_t e = dispatch_fused(ctx, L, &info, true);
+        if (e != cudaSuccess) { rc = (e == cudaErrorInvalidValue || e == cudaErrorLaunchOutOfResources) ? BANG_EINVAL : BANG_ECUDA; break; }
+    } while (0);
+    cudaFree(gl_dev);
+    if (rc != BANG_OK) { cudaGetLastError(); bang_destroy(ctx); return rc; }
+    *out = ctx;
+    return BANG_OK;
+}
+
+int bang_set_data(bang_ctx* ctx, const double* data_dev, const double* err_dev, const unsigned char* mask_dev) {
+    if (!ctx) return BANG_EINVAL;
+    if (!data_dev || !err_dev || !mask_dev) return fail(ctx, BANG_EINVAL, "bang_set_data: null pointer");
+    CU(cudaSetDevice(ctx->device));
+    double2* buf = nullptr;
+    const size_t n = (size_t)ctx->g.ny * 4 * ctx->nxp;
+    CU(cudaMalloc(&buf, n * sizeof(double2)));
+    k_prep_data<<<1, 1024, 0, ctx->stream>>>(ctx->g.nx, ctx->g.ny, ctx->nxp, data_dev, err_dev, mask_dev, buf, ctx->scal);
+    ctx->launches += 1;
+    double scal[2] = {0, 0};
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(scal, ctx->scal, sizeof(scal), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { cudaFree(buf); return fail(ctx, BANG_ECUDA, "bang_set_data: %s", cudaGetErrorString(e)); }
+    if (scal[1] != 0.0) {
+        cudaFree(buf);
+        return fail(ctx, BANG_EINVAL, "bang_set_data: %d used pixel(s) with err <= 0 or non-finite data/err", (int)scal[1]);
+    }
+    cudaFree(ctx->data);
+    ctx->data = buf; ctx->C0 = scal[0]; ctx->has_data = true;
+    return BANG_OK;
+}
+
+int bang_model_maps(bang_ctx* ctx, const double* theta_dev, int B, void* maps_dev) {
+    if (!ctx) return BANG_EINVAL;
+    if (B < 0 || (B > 0 && (!theta_dev || !maps_dev))) return fail(ctx, BANG_EINVAL, "bang_model_maps: bad arguments");
+    if (B == 0) return BANG_OK;
+    CU(cudaSetDevice(ctx->device));
+    FusedLaunch L = make_launch(ctx, theta_dev, B, 0, maps_dev, nullptr);
+    CU(dispatch_fused(ctx, L, nullptr, false));
+    ctx->launches += 1;
+    return BANG_OK;
+}
+
+int bang_loglike(bang_ctx* ctx, const double* theta_dev, int B, double* logL_dev) {
+    if (!ctx) return BANG_EINVAL;
+    if (B < 0 || (B > 0 && (!theta_dev || !logL_dev))) return fail(ctx, BANG_EINVAL, "bang_loglike: bad arguments");
+    if (!ctx->has_data) return fail(ctx, BANG_ENODATA, "bang_loglike: no data loaded");
+    if (B == 0) return BANG_OK;
+    CU(cudaSetDevice(ctx->device));
+    FusedLaunch L = make_launch(ctx, theta_dev, B, 1, nullptr, logL_dev);
+    CU(dispatch_fused(ctx, L, nullptr, false));
+    ctx->launches += 1;
+    return BANG_OK;
+}
+
+int bang_model_fine(bang_ctx* ctx, const double* theta_dev, int B, void* fine_dev) {
+    if (!ctx) return BANG_EINVAL;
+    if (B < 0 || (B > 0 && (!theta_dev || !fine_dev))) return fail(ctx, BANG_EINVAL, "bang_model_fine: bad arguments");
+    if (B == 0) return BANG_OK;
+    CU(cudaSetDevice(ctx->device));
+    const bool f64 = ctx->model.precision == BANG_FP64;
+    const int ctas = std::min(B, 8 * ctx->n_sm);
+    if (f64) {
+        FineParams<double> p{ctx->g, ctx->fit,
+                             PolyTab<double>{static_cast<const double*>(ctx->btab), ctx->btab_first, ctx->btab_cells},
+                             PolyTab<double>{static_cast<const double*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells},
+                             theta_dev, B, static_cast<double*>(fine_dev)};
+        const size_t smem = fused_smem_bytes<double>(0, 0);
+        CU(cudaFuncSetAttribute(k_fine<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k_fine<double><<<ctas, 256, smem, ctx->stream>>>(p);
+    } else {
+        FineParams<float> p{ctx->g, ctx->fit,
+                            PolyTab<float>{static_cast<const float*>(ctx->btab), ctx->btab_first, ctx->btab_cells},
+                            PolyTab<float>{static_cast<const float*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells},
+                            theta_dev, B, static_cast<float*>(fine_dev)};
+        const size_t smem = fused_smem_bytes<float>(0, 0);
+        CU(cudaFuncSetAttribute(k_fine<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k_fine<float><<<ctas, 256, smem, ctx->stream>>>(p);
+    }
+    ctx->launches += 1;
+    CU(cudaGetLastError());
+    return BANG_OK;
+}
+
+int bang_loglike_host(bang_ctx* ctx, const double* theta_host, int B, double* logL_host) {
+    if (!ctx) return BANG_EINVAL;
+    if (B < 0 || (B > 0 && (!theta_host || !logL_host))) return fail(ctx, BANG_EINVAL, "bang_loglike_host: bad arguments");
+    if (!ctx->has_data) return fail(ctx, BANG_ENODATA, "bang_loglike_host: no data loaded");
+    if (B == 0) return BANG_OK;
+    CU(cudaSetDevice(ctx->device));
+    int rc = ensure_staging(ctx, B, (size_t)B * sizeof(double));
+    if (rc != BANG_OK) return rc;
+    const size_t tb = (size_t)B * kNTheta * sizeof(double);
+    memcpy(ctx->h_theta, theta_host, tb);
+    CU(cudaMemcpyAsync(ctx->d_theta, ctx->h_theta, tb, cudaMemcpyHostToDevice, ctx->stream));
+    rc = bang_loglike(ctx, ctx->d_theta, B, static_cast<double*>(ctx->d_out));
+    if (rc != BANG_OK) return rc;
+    CU(cudaMemcpyAsync(ctx->h_out, ctx->d_out, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    memcpy(logL_host, ctx->h_out, (size_t)B * sizeof(double));
+    return BANG_OK;
+}
+
+int bang_model_maps_host(bang_ctx* ctx, const double* theta_host, int B, void* maps_host) {
+    if (!ctx) return BANG_EINVAL;
+    if (B < 0 || (B > 0 && (!theta_host || !maps_host))) return fail(ctx, BANG_EINVAL, "bang_model_maps_host: bad arguments");
+    if (B == 0) return BANG_OK;
+    CU(cudaSetDevice(ctx->device));
+    const size_t esz = ctx->model.precision == BANG_FP64 ? 8 : 4;
+    const size_t ob = (size_t)B * 4 * ctx->g.nx * ctx->g.ny * esz;
+    int rc = ensure_staging(ctx, B, ob);
+    if (rc != BANG_OK) return rc;
+    const size_t tb = (size_t)B * kNTheta * sizeof(double);
+    memcpy(ctx->h_theta, theta_host, tb);
+    CU(cudaMemcpyAsync(ctx->d_theta, ctx->h_theta, tb, cudaMemcpyHostToDevice, ctx->stream));
+    rc = bang_model_maps(ctx, ctx->d_theta, B, ctx->d_out);
+    if (rc != BANG_OK) return rc;
+    CU(cudaMemcpyAsync(ctx->h_out, ctx->d_out, ob, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    memcpy(maps_host, ctx->h_out, ob);
+    return BANG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,73 @@
+// bang_fused_inst.cu -- instantiations of the fused kernel for one (T, S); compiled once per pair with
+//   -DBANG_INST_T=float|double -DBANG_INST_TN=float|double -DBANG_INST_S=1..4
+// so that the heavy, fully unrolled PSF code builds in parallel translation units.
+#include "bang_host.h"
+
+#ifndef BANG_INST_T
+#error "compile with -DBANG_INST_T=<type> -DBANG_INST_TN=<name> -DBANG_INST_S=<s>"
+#endif
+
+namespace bang {
+namespace {
+
+template <typename T, int S, int NACC, int P>
+cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
+    auto kern = k_fused<T, S, NACC, P>;
+    const size_t smem = fused_smem_bytes<T>(S, L.nfb);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, L.threads, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    int ctas = L.ctas > 0 ? L.ctas : per_sm * L.n_sm;
+    if (ctas > L.B) ctas = L.B;
+    if (info) {
+        cudaFuncAttributes fa;
+        cudaFuncGetAttributes(&fa, kern);
+        info->regs = fa.numRegs; info->max_ctas_per_sm = per_sm; info->smem = smem; info->ctas = ctas;
+    }
+    if (query_only || L.B <= 0) return cudaSuccess;
+
+    FusedParams<T, S, NACC> p;
+    p.g = L.g; p.fit = L.fit;
+    p.btab = PolyTab<T>{static_cast<const T*>(L.btab), L.btab_first, L.btab_cells};
+    p.Ftab = PolyTab<T>{static_cast<const T*>(L.Ftab), L.Ftab_first, L.Ftab_cells};
+    for (int t = 0; t < NACC * S; ++t) p.W[t] = (T)L.W[t];
+    p.theta = L.theta; p.B = L.B; p.nxp = L.nxp; p.nfb = L.nfb; p.mode = L.mode;
+    p.maps = static_cast<T*>(L.maps); p.data = L.data; p.C0 = L.C0; p.logL = L.logL;
+    k_fused<T, S, NACC, P><<<ctas, L.threads, smem, L.stream>>>(p);
+    return cudaGetLastError();
+}
+
+template <typename T, int S, int P>
+cudaError_t launch_nacc(const FusedLaunch& L, FusedInfo* info, bool q) {
+    switch (L.nacc) {
+        case 1: return launch_one<T, S, 1, P>(L, info, q);
+        case 4: return launch_one<T, S, 4, P>(L, info, q);
+        case 7: return launch_one<T, S, 7, P>(L, info, q);
+        case 10: return launch_one<T, S, 10, P>(L, info, q);
+        case 13: return launch_one<T, S, 13, P>(L, info, q);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace
+
+#define BANG_CAT3(a, b, c) a##b##_##c
+#define BANG_NAME(tn, s) BANG_CAT3(launch_fused_, tn, s)
+
+cudaError_t BANG_NAME(BANG_INST_TN, BANG_INST_S)(const FusedLaunch& L, FusedInfo* info, bool query_only) {
+    using T = BANG_INST_T;
+    constexpr int S = BANG_INST_S;
+    if (L.g.s != S) return cudaErrorInvalidValue;
+    if constexpr (sizeof(T) == 8) {
+        if (L.P == 2) return launch_nacc<T, S, 2>(L, info, query_only);
+    } else {
+        if (L.P == 4) return launch_nacc<T, S, 4>(L, info, query_only);
+        if (L.P == 2) return launch_nacc<T, S, 2>(L, info, query_only);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace bang

@@ -1,0 +1,545 @@
+// bang_kernels.cuh -- the hot path: per-theta decode + radial table (a0, a1), per-fine-cell model (a2, a3), separable
+// PSF fused with the rebin (a4, a5) and the masked chi-square reduction (a6), in ONE persistent kernel per batch.
+// Step names are those of SURVEY.md sec. 8(a) / DESIGN.md "The path".  T = float (BANG_FP32) or double (BANG_FP64).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "bang_math.cuh"
+
+namespace bang {
+
+constexpr int kNTheta = 17;      // Table 1
+constexpr int kMaxOct = 64;          // octaves of r^2 the per-theta v_c table may span
+constexpr unsigned C_BULGE = 1u, C_DISC1 = 2u, C_DISC2 = 4u, C_HALO = 8u;
+constexpr int kBulgeOctLo = -44, kBulgeOctHi = 36;    // universal bulge tables: s^2 in [2^-44, 2^36)
+constexpr int kFOctLo = -60, kFOctHi = 10;            // universal Freeman table: y^2 in [2^-60, 2^10)
+
+// ---- fast fp32 special-function-unit ops (MUFU), and their fp64 counterparts -------------------------------------
+BANG_D float fast_rsqrt(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+BANG_D float fast_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+BANG_D float fast_sqrt(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+BANG_D float fast_exp2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+BANG_D double fast_rsqrt(double x) { return 1.0 / sqrt(x); }
+BANG_D double fast_rcp(double x) { return 1.0 / x; }
+BANG_D double fast_sqrt(double x) { return sqrt(x); }
+BANG_D double fast_exp2(double x) { return exp2(x); }
+
+// ---- a piecewise-polynomial table in global or shared memory -----------------------------------------------------
+template <typename T>
+struct PolyTab {
+    const T* coef;    // [n_cells][n_func][D+1], monomial coefficients in t in [-1,1)
+    int first;        // global interval number (tab_cell) of coef[0]
+    int n_cells;
+};
+
+template <typename T, int D>
+BANG_D T horner(const T* c, T t) {
+    T v = c[D];
+#pragma unroll
+    for (int d = D - 1; d >= 0; --d) v = fma(v, t, c[d]);
+    return v;
+}
+
+// ---- per-theta constants (a0), decoded once per theta in fp64 by one thread ----------------------------------------
+struct ThetaD {      // what the table build needs, in double
+    double GMb, Rb;              // bulge v_c^2 = GMb r/(r+Rb)^2  (eq. 2)
+    double Ad[2], inv2Rd[2];     // disc  v_c^2 = Ad F(r inv2Rd),  Ad = 2 G M_d/R_d  (eq. 9, reading D)
+    double Ah, hs;               // halo: Hernquist GMh, Rh;  NFW: G M200/mu(c), 1/r_s  (reading H)
+};
+template <typename T>
+struct ThetaC {
+    int valid;
+    int jcx, jcy;                // fine cell (buffer coordinates) nearest to the galaxy centre
+    int vfirst, vcells;          // per-theta v_c table: first global interval, number of intervals
+    T hc, hs;                    // h cos PA, h sin PA   (h = fine cell size in kpc)
+    T xp0, yp0;                  // rotated offset of cell (jcx, jcy) from the centre
+    T inv_ci2;                   // 1/cos^2 i
+    T invRb2, ampBb, ampIb, MLb; // bulge: s^2 = R^2 invRb2;  B_b = ampBb SigmaTilde;  B_b sigma_b^2 = ampIb J
+    T cexp[2], ampBd[2], MLd[2]; // disc j: B_d = ampBd 2^(r cexp)
+    T vk[2], q3[2];              // -sin i k_j   and   (1 - k_j^2)/3
+    ThetaD d;
+};
+
+// geometry of the run, the same for every theta (built on the host at bang_create)
+struct GridC {
+    int nx, ny, s, rk;
+    int nfx, nfy;                // evaluated fine cells: n s + 2 r_k (buffer coordinates 0..nf-1)
+    double jsx, jsy;             // buffer index of the sky origin: r_k - 1/2 + n s/2
+    double spx;                  // s / pix_arcsec: fine cells per arcsec
+    double h;                    // fine cell size [kpc]
+    unsigned comps;
+    int halo_profile;
+};
+
+struct FitC {                    // Chebyshev-node fit of degree D: nodes t_k and the inverse Vandermonde matrix
+    double tnode[8];
+    double vinv[64];             // vinv[d*(D+1)+k]: coefficient d = sum_k vinv[d][k] f(t_k)
+};
+
+// Freeman-disc function from the universal table (y^2 in [2^-60, 2^10)), its leading small-y form, and the
+// large-argument expansion (DLMF 10.40.6) beyond.
+template <typename T>
+BANG_D double freeman_F_tab(const PolyTab<T>& Ftab, double y2) {
+    if (y2 >= 1024.0) {
+        const double iz2 = 0.25 / y2;
+        double a0 = 1.0, a1 = 1.0, sum = 0.0;
+#pragma unroll 1
+        for (int k = 1; k < 14; ++k) {
+            const double odd = 2.0 * k - 1.0;
+            const double f = -(odd / (2.0 * k)) * iz2;
+            a0 *= f * (0.0 - odd * odd);
+            a1 *= f * (4.0 - odd * odd);
+            sum += a0 - a1;
+        }
+        return 0.5 * sqrt(y2) * sum;
+    }
+    if (y2 < 8.673617379884035e-19)     // 2^-60: F = y^2 [-ln(y/2) - gamma - 1/2] (1 + O(y^2 ln y))
+        return y2 * (-0.5 * log(0.25 * y2) - kEulerGamma - 0.5);
+    T t;
+    const int c = min(max(tab_cell((T)y2, t) - Ftab.first, 0), Ftab.n_cells - 1);
+    return (double)horner<T, TabCfg<T>::D>(Ftab.coef + (size_t)c * (TabCfg<T>::D + 1), t);
+}
+
+// total circular speed squared at radius r in the disc plane (eq. 10)
+template <typename T>
+BANG_D double vc2_total(const ThetaD& d, const GridC& g, const PolyTab<T>& Ftab, double r) {
+    double v2 = 0.0;
+    if (g.comps & C_BULGE) { const double a = r + d.Rb; v2 += d.GMb * r / (a * a); }
+#pragma unroll
+    for (int j = 0; j < 2; ++j)
+        if (g.comps & (j ? C_DISC2 : C_DISC1)) {
+            const double y = r * d.inv2Rd[j];
+            v2 += d.Ad[j] * freeman_F_tab(Ftab, y * y);
+        }
+    if (g.comps & C_HALO) {
+        if (g.halo_profile == 1) v2 += d.Ah * nfw_mu<double>(r * d.hs) / r;
+        else { const double a = r + d.hs; v2 += d.Ah * r / (a * a); }
+    }
+    return v2;
+}
+
+// a0: decode theta[17] (Table 1).  Run by ONE thread; everything in fp64.
+template <typename T>
+BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, ThetaC<T>& c) {
+    const unsigned comps = g.comps;
+    c.valid = 0;
+    bool ok = isfinite(th[0]) && isfinite(th[1]) && isfinite(th[2]) && isfinite(th[3]) && fabs(th[3]) < 90.0;
+    if (comps & C_BULGE) ok = ok && isfinite(th[4]) && th[5] > 0 && isfinite(th[5]) && th[12] > 0 && isfinite(th[12]);
+    for (int j = 0; j < 2; ++j)
+        if (comps & (j ? C_DISC2 : C_DISC1))
+            ok = ok && isfinite(th[6 + 2 * j]) && th[7 + 2 * j] > 0 && isfinite(th[7 + 2 * j]) && th[13 + j] > 0 &&
+                 isfinite(th[13 + j]) && fabs(th[15 + j]) <= 1.0;
+    if (comps & C_HALO) ok = ok && isfinite(th[10]) && th[11] > 0 && isfinite(th[11]);
+    if (!ok) return;
+
+    // sec. 2.1 (fn 2 at :68): centre, position angle (counter-clockwise from +x), inclination
+    double sp, cp, si, ci;
+    sincos(th[2] * (kPi / 180.0), &sp, &cp);
+    sincos(th[3] * (kPi / 180.0), &si, &ci);
+    const double h = g.h;
+    const double Jsx = g.jsx + th[0] * g.spx, Jsy = g.jsy + th[1] * g.spx;      // fractional buffer index of the centre
+    const int jcx = (int)fmin(fmax(rint(Jsx), 0.0), (double)(g.nfx - 1));
+    const int jcy = (int)fmin(fmax(rint(Jsy), 0.0), (double)(g.nfy - 1));
+    const double dx = (jcx - Jsx) * h, dy = (jcy - Jsy) * h;                    // offset of that cell from the centre [kpc]
+    c.jcx = jcx; c.jcy = jcy;
+    c.hc = (T)(h * cp); c.hs = (T)(h * sp);
+    c.xp0 = (T)(dx * cp + dy * sp);
+    c.yp0 = (T)(-dx * sp + dy * cp);
+    const double inv_ci2 = 1.0 / (ci * ci);
+    c.inv_ci2 = (T)inv_ci2;
+
+    // range of radii on this theta's grid: R^2 >= dx^2+dy^2 (attained at the nearest cell); maxima at the corners
+    const double floor2 = ldexp(1.0, 2 * kRFloorLog2);
+    const double R2min = fmax(dx * dx + dy * dy, floor2);
+    double R2max = 0.0, r2max = 0.0;
+    for (int k = 0; k < 4; ++k) {
+        const double a = ((k & 1) ? g.nfx - 1 : 0) - Jsx, b = ((k & 2) ? g.nfy - 1 : 0) - Jsy;
+        const double X = a * h, Y = b * h;
+        const double xp = X * cp + Y * sp, yp = -X * sp + Y * cp;
+        R2max = fmax(R2max, xp * xp + yp * yp);
+        r2max = fmax(r2max, xp * xp + yp * yp * inv_ci2);
+    }
+    R2max = fmax(R2max, floor2); r2max = fmax(r2max, floor2);
+    const double lo_m = 1.0 - 0x1p-10, hi_m = 1.0 + 0x1p-10;
+    const int e_lo = ilogb(R2min * lo_m), e_hi = ilogb(r2max * hi_m);
+    if (e_hi - e_lo + 1 > kMaxOct || e_hi > 120) return;
+    c.vfirst = tab_first_cell<T>(e_lo);
+    c.vcells = (e_hi - e_lo + 1) << TabCfg<T>::M;
+
+    ThetaD& d = c.d;
+    // bulge: eq. 1-6
+    c.invRb2 = T(1); c.ampBb = T(0); c.ampIb = T(0); c.MLb = T(1);
+    d.GMb = 0.0; d.Rb = 1.0;
+    if (comps & C_BULGE) {
+        const double Mb = exp10(th[4]), Rb = th[5], MLb = th[12];
+        const double inv = 1.0 / (Rb * Rb);
+        if (!(R2min * inv * lo_m >= ldexp(1.0, kBulgeOctLo)) || !(R2max * inv * hi_m < ldexp(1.0, kBulgeOctHi))) return;
+        c.invRb2 = (T)inv;
+        c.ampBb = (T)(Mb / (2.0 * kPi * Rb * Rb) / MLb * 1e-6);                          // eq. 4, in Lsun/pc^2
+        c.ampIb = (T)(kG * Mb * Mb / (2.0 * kPi * Rb * Rb * Rb) * 2.0 / MLb * 1e-6);     // eq. 6 first form
+        c.MLb = (T)MLb;
+        d.GMb = kG * Mb; d.Rb = Rb;
+    }
+    // discs: eq. 7-9, 11-12
+    for (int j = 0; j < 2; ++j) {
+        c.cexp[j] = T(0); c.ampBd[j] = T(0); c.MLd[j] = T(1); c.vk[j] = T(0); c.q3[j] = T(0);
+        d.Ad[j] = 0.0; d.inv2Rd[j] = 1.0;
+        if (comps & (j ? C_DISC2 : C_DISC1)) {
+            const double Md = exp10(th[6 + 2 * j]), Rd = th[7 + 2 * j], ML = th[13 + j], k = th[15 + j];
+            c.cexp[j] = (T)(-1.4426950408889634 / Rd);
+            c.ampBd[j] = (T)(Md / (2.0 * kPi * Rd * Rd * ci) / ML * 1e-6);               // eq. 7-8
+            c.MLd[j] = (T)ML;
+            c.vk[j] = (T)(-si * k);                                                      // eq. 11
+            c.q3[j] = (T)((1.0 - k * k) / 3.0);                                          // eq. 12
+            d.Ad[j] = 2.0 * kG * Md / Rd;
+            d.inv2Rd[j] = 0.5 / Rd;
+        }
+    }
+    // halo (reading H)
+    d.Ah = 0.0; d.hs = 1.0;
+    if (comps & C_HALO) {
+        const double Mh = exp10(th[10]);
+        if (g.halo_profile == 1) {
+            const double cc = th[11];
+            d.Ah = kG * Mh / nfw_mu<double>(cc);
+            d.hs = cc / nfw_r200(Mh);
+        } else {
+            d.Ah = kG * Mh; d.hs = th[11];
+        }
+    }
+    c.valid = 1;
+}
+
+// a1: the per-theta radial table v_c(r), a piecewise polynomial in u = r^2 on the pseudo-log grid, built cooperatively
+// by the CTA in shared memory: every thread evaluates v_c at Chebyshev nodes (fp64), then one thread per interval turns
+// its D+1 node values into monomial coefficients.  Must be called by all threads; ends with a __syncthreads().
+template <typename T>
+BANG_D void build_vc_table(const ThetaC<T>& c, const GridC& g, const FitC& fit, const PolyTab<T>& Ftab, T* vtab) {
+    constexpr int D = TabCfg<T>::D, NC = D + 1;
+    const int n = c.vcells * NC;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const int cell = i / NC, k = i - cell * NC;
+        double lo, width;
+        tab_interval<T>(c.vfirst + cell, lo, width);
+        const double u = lo + 0.5 * width * (fit.tnode[k] + 1.0);
+        vtab[i] = (T)sqrt(vc2_total(c.d, g, Ftab, sqrt(u)));
+    }
+    __syncthreads();
+    for (int cell = threadIdx.x; cell < c.vcells; cell += blockDim.x) {
+        T* p = vtab + cell * NC;
+        double f[NC], co[NC];
+#pragma unroll
+        for (int k = 0; k < NC; ++k) f[k] = (double)p[k];
+#pragma unroll
+        for (int d = 0; d < NC; ++d) {
+            double a = 0.0;
+#pragma unroll
+            for (int k = 0; k < NC; ++k) a = fma(fit.vinv[d * NC + k], f[k], a);
+            co[d] = a;
+        }
+#pragma unroll
+        for (int d = 0; d < NC; ++d) p[d] = (T)co[d];
+    }
+    __syncthreads();
+}
+
+// a2 + a3: one fine cell (buffer coordinates jx, jy) -> B_tot, v_los, sigma_los, <L/M>   (eqs. 4-15, 19)
+template <typename T>
+BANG_D void eval_cell(const ThetaC<T>& c, const unsigned comps, const PolyTab<T>& btab, const T* __restrict__ vtab,
+                      int jx, int jy, T& oB, T& oV, T& oS, T& oLM) {
+    constexpr int D = TabCfg<T>::D, NC = D + 1;
+    // sec. 2.1: rotate into the galaxy frame (fn 2); R on the sky (bulge), r in the disc plane
+    const T a = (T)(jx - c.jcx), b = (T)(jy - c.jcy);
+    const T xp = fma(a, c.hc, fma(b, c.hs, c.xp0));
+    const T yp = fma(b, c.hc, fma(-a, c.hs, c.yp0));
+    const T floor2 = sizeof(T) == 4 ? T(0x1p-32f) : T(0x1p-32);
+    const T y2 = yp * yp;
+    const T R2 = fmax(fma(xp, xp, y2), floor2);
+    const T r2 = fmax(fma(xp, xp, y2 * c.inv_ci2), floor2);
+    const T rinv = fast_rsqrt(r2);
+    const T r = r2 * rinv;
+    const T cosphi = xp * rinv;
+
+    // bulge: Sigma_b (eq. 4) and Sigma_b sigma_b^2 (eq. 6) from the scale-free tables at s^2 = R^2/R_b^2
+    T Bb = T(0), IbL = T(0);
+    if (comps & C_BULGE) {
+        T t;
+        const int cell = (int)min((unsigned)(tab_cell(R2 * c.invRb2, t) - btab.first), (unsigned)(btab.n_cells - 1));
+        const T* p = btab.coef + (size_t)cell * (2 * NC);
+        T cs[NC], cj[NC];
+        if constexpr (sizeof(T) == 4) {
+            const float4 v0 = __ldg(reinterpret_cast<const float4*>(p));
+            const float4 v1 = __ldg(reinterpret_cast<const float4*>(p) + 1);
+            cs[0] = v0.x; cs[1] = v0.y; cs[2] = v0.z; cs[3] = v0.w;
+            cj[0] = v1.x; cj[1] = v1.y; cj[2] = v1.z; cj[3] = v1.w;
+        } else {
+#pragma unroll
+            for (int d = 0; d < NC; d += 2) {
+                const double2 v0 = __ldg(reinterpret_cast<const double2*>(p + d));
+                const double2 v1 = __ldg(reinterpret_cast<const double2*>(p + NC + d));
+                cs[d] = v0.x; cs[d + 1] = v0.y; cj[d] = v1.x; cj[d + 1] = v1.y;
+            }
+        }
+        Bb = c.ampBb * horner<T, D>(cs, t);
+        IbL = c.ampIb * horner<T, D>(cj, t);
+    }
+    // discs: eq. 7-8.  Without a bulge the two exponentials are scaled by the larger one so that the ratios below
+    // survive fp32 underflow far outside small discs.
+    const T e1a = r * c.cexp[0], e2a = r * c.cexp[1];
+    T shift = T(0);
+    if (!(comps & C_BULGE)) {
+        shift = (comps & C_DISC1) ? ((comps & C_DISC2) ? fmax(e1a, e2a) : e1a) : e2a;
+    }
+    const T Bd1 = c.ampBd[0] * fast_exp2(e1a - shift);
+    const T Bd2 = c.ampBd[1] * fast_exp2(e2a - shift);
+    // v_c(r) from the per-theta table (eq. 10)
+    T vc;
+    {
+        T t;
+        const int cell = (int)min((unsigned)(tab_cell(r2, t) - c.vfirst), (unsigned)(c.vcells - 1));
+        const T* p = vtab + cell * NC;
+        T cv[NC];
+        if constexpr (sizeof(T) == 4) {
+            const float4 v0 = *reinterpret_cast<const float4*>(p);
+            cv[0] = v0.x; cv[1] = v0.y; cv[2] = v0.z; cv[3] = v0.w;
+        } else {
+#pragma unroll
+            for (int d = 0; d < NC; d += 2) {
+                const double2 v0 = *reinterpret_cast<const double2*>(p + d);
+                cv[d] = v0.x; cv[d + 1] = v0.y;
+            }
+        }
+        vc = horner<T, D>(cv, t);
+    }
+    // eq. 13, 14 (with 11), 15 (with 12), 19
+    const T Btot = Bb + Bd1 + Bd2;
+    const T Stot = fma(c.MLb, Bb, fma(c.MLd[0], Bd1, c.MLd[1] * Bd2));     // total mass surface density (x 1e-6)
+    const T invB = fast_rcp(Btot);
+    const T kB = fma(c.vk[0], Bd1, c.vk[1] * Bd2);
+    const T qB = fma(c.q3[0], Bd1, c.q3[1] * Bd2);
+    oV = cosphi * vc * kB * invB;
+    oS = fast_sqrt(fma(vc * vc, qB, IbL) * invB);
+    oLM = Btot * fast_rcp(Stot);
+    oB = (comps & C_BULGE) ? Btot : Btot * fast_exp2(shift);
+}
+
+// ---- the fused kernel ---------------------------------------------------------------------------------------------
+template <typename T, int S, int NACC>
+struct FusedParams {
+    GridC g;
+    FitC fit;
+    PolyTab<T> btab, Ftab;
+    T W[NACC * S];               // composite x s box (*) Gaussian taps, zero padded (a4 + a5)
+    const double* theta;         // [B][17]
+    int B;
+    int nxp;                     // data columns padded to a multiple of P
+    int nfb;                     // row-buffer width in cells (>= (nxp-1+NACC) S, multiple of 4, plus over-read slack)
+    int mode;                    // 0: write maps, 1: reduce the likelihood
+    T* maps;                     // [B][4][ny][nx]
+    const double2* data;         // [ny][4][nxp] {d, 1/e} (1/e = 0 where masked or padded)
+    double C0;                   // sum over used pixels of -1/2 ln(2 pi e^2)
+    double* logL;                // [B]
+};
+
+template <typename T>
+inline size_t fused_smem_bytes(int S, int nfb) {
+    return (sizeof(ThetaC<T>) + 15) / 16 * 16 + (size_t)kMaxOct * (1 << TabCfg<T>::M) * (TabCfg<T>::D + 1) * sizeof(T) +
+           (size_t)S * 4 * nfb * sizeof(T) + 32 * sizeof(double);
+}
+
+// N consecutive values from shared memory into registers with the widest vector loads the alignment ALIGN (bytes)
+// allows; may read up to one vector past N (the row buffer carries that slack).
+template <typename T, int N, int ALIGN>
+BANG_D void load_run(const T* __restrict__ src, T (&f)[N]) {
+    constexpr int V = ALIGN / (int)sizeof(T);
+    if constexpr (V == 4) {
+#pragma unroll
+        for (int i = 0; i < N; i += 4) {
+            const float4 v = *reinterpret_cast<const float4*>(src + i);
+            f[i] = v.x;
+            if (i + 1 < N) f[i + 1] = v.y;
+            if (i + 2 < N) f[i + 2] = v.z;
+            if (i + 3 < N) f[i + 3] = v.w;
+        }
+    } else if constexpr (V == 2 && sizeof(T) == 4) {
+#pragma unroll
+        for (int i = 0; i < N; i += 2) {
+            const float2 v = *reinterpret_cast<const float2*>(src + i);
+            f[i] = v.x;
+            if (i + 1 < N) f[i + 1] = v.y;
+        }
+    } else if constexpr (V == 2 && sizeof(T) == 8) {
+#pragma unroll
+        for (int i = 0; i < N; i += 2) {
+            const double2 v = *reinterpret_cast<const double2*>(src + i);
+            f[i] = v.x;
+            if (i + 1 < N) f[i + 1] = v.y;
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < N; ++i) f[i] = src[i];
+    }
+}
+
+template <typename T, int S, int NACC, int P>
+__global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
+    constexpr int D = TabCfg<T>::D, NC = D + 1;
+    constexpr int RUN = (P - 1 + NACC) * S;          // fine cells one thread reads per row for its P data pixels
+    constexpr int RUN_BYTES = P * S * (int)sizeof(T);   // byte stride between the runs of neighbouring threads
+    constexpr int ALIGN = RUN_BYTES % 16 == 0 ? 16 : (RUN_BYTES % 8 == 0 ? 8 : (int)sizeof(T));
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    ThetaC<T>& c = *reinterpret_cast<ThetaC<T>*>(smem_raw);
+    constexpr size_t off_tab = (sizeof(ThetaC<T>) + 15) / 16 * 16;
+    T* vtab = reinterpret_cast<T*>(smem_raw + off_tab);
+    T* rowbuf = vtab + (size_t)kMaxOct * (1 << TabCfg<T>::M) * NC;
+    const int nfb = p.nfb;
+    double* red = reinterpret_cast<double*>(rowbuf + (size_t)S * 4 * nfb);
+
+    const GridC& g = p.g;
+    const int tid = threadIdx.x, NT = blockDim.x;
+    const int G = p.nxp / P;                         // pixel groups per map
+    const int items = 4 * G;
+    const int q = tid / G, grp = tid - q * G;        // this thread's observable and pixel group in the PSF phase
+    const int nsuper = g.ny + NACC - 1;
+    const int ncell_sr = S * g.nfx;                  // cells evaluated per super-row
+    const size_t npix = (size_t)g.nx * g.ny;
+
+    for (int i = tid; i < S * 4 * nfb; i += NT) rowbuf[i] = T(0);
+
+    for (int b = blockIdx.x; b < p.B; b += gridDim.x) {
+        __syncthreads();
+        if (tid == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, c);
+        __syncthreads();
+        if (!c.valid) {                              // out-of-domain theta: NaN maps / -inf likelihood
+            if (p.mode == 0) {
+                const T qnan = (T)nan("");
+                for (size_t i = tid; i < 4 * npix; i += NT) p.maps[(size_t)b * 4 * npix + i] = qnan;
+            } else if (tid == 0) {
+                p.logL[b] = -INFINITY;
+            }
+            continue;
+        }
+        build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
+
+        T acc[P][NACC];
+#pragma unroll
+        for (int i = 0; i < P; ++i)
+#pragma unroll
+            for (int k = 0; k < NACC; ++k) acc[i][k] = T(0);
+        double chi2 = 0.0;
+
+        for (int sr = 0; sr < nsuper; ++sr) {
+            // ---- a2 + a3: evaluate the S fine rows of this super-row into shared memory
+            {
+                int j = 0, x = tid;
+                while (x >= g.nfx) { x -= g.nfx; ++j; }
+                for (int i = tid; i < ncell_sr; i += NT) {
+                    const int jy = sr * S + j;
+                    T vB = T(0), vV = T(0), vS = T(0), vL = T(0);
+                    if (jy < g.nfy) eval_cell<T>(c, g.comps, p.btab, vtab, x, jy, vB, vV, vS, vL);
+                    T* dst = rowbuf + (size_t)(j * 4) * nfb + x;
+                    dst[0] = vB; dst[nfb] = vV; dst[2 * nfb] = vS; dst[3 * nfb] = vL;
+                    x += NT;
+                    while (x >= g.nfx) { x -= g.nfx; ++j; }
+                }
+            }
+            __syncthreads();
+            // ---- a4 + a5: PSF along x fused with the rebin, then scattered along y into the running data rows
+            if (tid < items) {
+#pragma unroll
+                for (int j = 0; j < S; ++j) {
+                    T f[RUN];
+                    load_run<T, RUN, ALIGN>(rowbuf + (size_t)(j * 4 + q) * nfb + grp * (P * S), f);
+#pragma unroll
+                    for (int i = 0; i < P; ++i) {
+                        T xp = T(0);
+#pragma unroll
+                        for (int t = 0; t < NACC * S; ++t) xp = fma(p.W[t], f[i * S + t], xp);
+#pragma unroll
+                        for (int k = 0; k < NACC; ++k) acc[i][k] = fma(p.W[(NACC - 1 - k) * S + j], xp, acc[i][k]);
+                    }
+                }
+                // ---- a6 (or map output): data row py is complete
+                const int py = sr - (NACC - 1);
+                if (py >= 0) {
+#pragma unroll
+                    for (int i = 0; i < P; ++i) {
+                        const int px = grp * P + i;
+                        T m = acc[i][0];
+                        if (q == 3) m = T(1) / m;                      // M/L = 1/<L/M> (fn 10)
+                        if (px < g.nx) {
+                            if (p.mode == 0) {
+                                p.maps[((size_t)b * 4 + q) * npix + (size_t)py * g.nx + px] = m;
+                            } else {
+                                const double2 de = __ldg(p.data + ((size_t)py * 4 + q) * p.nxp + px);
+                                const double z = (de.x - (double)m) * de.y;   // eq. 18, residual in fp64
+                                chi2 = fma(z, z, chi2);
+                            }
+                        }
+                    }
+                }
+#pragma unroll
+                for (int i = 0; i < P; ++i) {
+#pragma unroll
+                    for (int k = 0; k + 1 < NACC; ++k) acc[i][k] = acc[i][k + 1];
+                    acc[i][NACC - 1] = T(0);
+                }
+            }
+            __syncthreads();
+        }
+        if (p.mode == 1) {                           // a6: block reduction, warp shuffles, fp64
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) chi2 += __shfl_xor_sync(0xffffffffu, chi2, o);
+            if ((tid & 31) == 0) red[tid >> 5] = chi2;
+            __syncthreads();
+            if (tid == 0) {
+                double s = 0.0;
+                for (int w = 0; w < (NT + 31) / 32; ++w) s += red[w];
+                p.logL[b] = p.C0 - 0.5 * s;
+            }
+        }
+    }
+}
+
+// un-convolved fine maps (bang_model_fine): one CTA per theta, same decode / table / cell code as the fused kernel
+template <typename T>
+struct FineParams {
+    GridC g;
+    FitC fit;
+    PolyTab<T> btab, Ftab;
+    const double* theta;
+    int B;
+    T* fine;                     // [B][4][nfy][nfx]
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_fine(const __grid_constant__ FineParams<T> p) {
+    constexpr int NC = TabCfg<T>::D + 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    ThetaC<T>& c = *reinterpret_cast<ThetaC<T>*>(smem_raw);
+    constexpr size_t off_tab = (sizeof(ThetaC<T>) + 15) / 16 * 16;
+    T* vtab = reinterpret_cast<T*>(smem_raw + off_tab);
+    (void)NC;
+    const GridC& g = p.g;
+    const size_t plane = (size_t)g.nfx * g.nfy;
+    for (int b = blockIdx.x; b < p.B; b += gridDim.x) {
+        __syncthreads();
+        if (threadIdx.x == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, c);
+        __syncthreads();
+        T* out = p.fine + (size_t)b * 4 * plane;
+        if (!c.valid) {
+            const T qnan = (T)nan("");
+            for (size_t i = threadIdx.x; i < 4 * plane; i += blockDim.x) out[i] = qnan;
+            continue;
+        }
+        build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
+        for (size_t i = threadIdx.x; i < plane; i += blockDim.x) {
+            const int jy = (int)(i / g.nfx), jx = (int)(i - (size_t)jy * g.nfx);
+            T vB, vV, vS, vL;
+            eval_cell<T>(c, g.comps, p.btab, vtab, jx, jy, vB, vV, vS, vL);
+            out[i] = vB; out[plane + i] = vV; out[2 * plane + i] = vS; out[3 * plane + i] = vL;
+        }
+    }
+}
+
+}  // namespace bang
