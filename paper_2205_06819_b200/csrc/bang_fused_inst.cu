@@ -1,6 +1,9 @@
 // bang_fused_inst.cu -- instantiations of the fused kernel for one (T, S); compiled once per pair with
 //   -DBANG_INST_T=float|double -DBANG_INST_TN=float|double -DBANG_INST_S=1..4
 // so that the heavy, fully unrolled PSF code builds in parallel translation units.
+#include <cstdio>
+#include <cstdlib>
+
 #include "bang_host.h"
 
 #ifndef BANG_INST_T
@@ -28,6 +31,12 @@ cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
         info->regs = fa.numRegs; info->max_ctas_per_sm = per_sm; info->smem = smem; info->ctas = ctas;
     }
     if (query_only || L.B <= 0) return cudaSuccess;
+    if (getenv("BANG_VERBOSE")) {
+        cudaFuncAttributes fa;
+        cudaFuncGetAttributes(&fa, kern);
+        fprintf(stderr, "[bang] k_fused<%s,S=%d,NACC=%d,P=%d> regs=%d smem=%zu threads=%d ctas/SM=%d grid=%d B=%d\n",
+                sizeof(T) == 4 ? "f32" : "f64", S, NACC, P, fa.numRegs, smem, L.threads, per_sm, ctas, L.B);
+    }
 
     FusedParams<T, S, NACC> p;
     p.g = L.g; p.fit = L.fit;

@@ -1,0 +1,61 @@
+"""Multi-GPU plumbing: theta vectors are independent, so the batch is sharded across ranks
+with no data-path collective; grid, PSF, data, errors and mask (<= 1.5 MB) are replicated.  The only exchanges are
+the max-over-ranks of the device time and the gather of logL, both through torch.distributed (NCCL on GPUs,
+gloo in the CPU tests).  Nothing here computes any part of the model."""
+from __future__ import annotations
+
+import os
+
+import numpy as np
+
+
+def env_rank_world():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+
+
+def shard_bounds(B: int, rank: int, world: int):
+    """Contiguous, balanced [lo, hi) of rank's shard of a batch of B (the first B % world ranks get one more)."""
+    base, rem = divmod(B, world)
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+def shard(theta: np.ndarray, rank: int, world: int) -> np.ndarray:
+    lo, hi = shard_bounds(theta.shape[0], rank, world)
+    return theta[lo:hi]
+
+
+def max_over_ranks(value: float, device=None) -> float:
+    """max of a per-rank scalar (device time); identity when torch.distributed is not initialised."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(value)
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(value: float, device=None) -> float:
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(value)
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def gather_logl(local, B: int, rank: int, world: int):
+    """All-gather the per-rank logL shards (torch tensors) into the full [B] vector, in batch order."""
+    import torch
+    import torch.distributed as dist
+    if world == 1 or not (dist.is_available() and dist.is_initialized()):
+        return local
+    sizes = [shard_bounds(B, r, world)[1] - shard_bounds(B, r, world)[0] for r in range(world)]
+    pad = max(sizes)
+    buf = torch.zeros(pad, dtype=local.dtype, device=local.device)
+    buf[: local.numel()] = local
+    out = [torch.empty_like(buf) for _ in range(world)]
+    dist.all_gather(out, buf)
+    return torch.cat([o[:n] for o, n in zip(out, sizes)])

@@ -83,9 +83,13 @@ def near_truth_slots(idx: int, B: int) -> np.ndarray:
     return np.sort(rng.choice(B, size=n, replace=False))
 
 
+LOG_MASS_SLOTS = [4, 6, 8, 10]          # theta entries that hold log10 of a mass
+
+
 def theta_batch(idx: int, B: int | None = None) -> np.ndarray:
-    """[B][17] parameter vectors: uniform in the prior box, with 16 vectors within +-1 % of theta_true
-    (additive +-0.01 arcsec on the centre, +-0.1 deg on the angles) at seeded slots.  Config 1: theta_true."""
+    """[B][17] parameter vectors: uniform in the prior box, with 16 vectors within +-1 % of theta_true at seeded
+    slots (reading Q): +-1 % on every physical quantity (masses, not their logarithms: log10 M +- log10(1.01)),
+    additive +-0.01 arcsec on the centre and +-0.1 deg on the angles.  Config 1: theta_true."""
     cfg = CONFIGS[idx]
     B = cfg["B"] if B is None else B
     if idx == 1:
@@ -96,6 +100,7 @@ def theta_batch(idx: int, B: int | None = None) -> np.ndarray:
     slots = near_truth_slots(idx, B)
     u = rng.uniform(-1.0, 1.0, size=(len(slots), NTHETA))
     near = tt * (1.0 + 0.01 * u)
+    near[:, LOG_MASS_SLOTS] = tt[LOG_MASS_SLOTS] + np.log10(1.0 + 0.01 * u[:, LOG_MASS_SLOTS])
     near[:, 0:2] = tt[0:2] + 0.01 * u[:, 0:2]
     near[:, 2:4] = tt[2:4] + 0.1 * u[:, 2:4]
     near[:, 15:17] = np.clip(near[:, 15:17], -1.0, 1.0)

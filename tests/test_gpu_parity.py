@@ -1,0 +1,219 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the fp64 CPU oracle, element by
+element on the same seeded inputs, for the five BASELINE.json configs, plus properties that hold at full size.
+
+Tolerances (BASELINE.json north_star; readings P and Q), written out here:
+  maps, fp64 mode: |g-o| <= 1e-9 |o| per pixel;  fp32 mode: <= 1e-4 |o|;
+        v_los crosses zero, so its denominator is max(|o|, 1e-3 max_map|o|) (reading P);
+        fp32 B: plus an absolute floor of 1e-30 (fp32 cannot hold the oracle's values below ~1e-38);
+  logL, fp32 mode: |dlogL| <= 1e-3 sqrt(N_pix) for the near-truth theta (N_pix = used spaxels per map), and for every
+        theta the first-order bound implied by the per-pixel tolerance, |dlogL| <= 1e-4 sum_p |z_p| |m_p| / e_p;
+  logL, fp64 mode: the same first-order bound with 1e-9.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2205_06819_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+RTOL = {"fp64": 1e-9, "fp32": 1e-4}
+
+
+@pytest.fixture(scope="module")
+def bang():
+    import torch
+    assert torch.cuda.is_available(), "the -m gpu tests need a CUDA device"
+    from paper_2205_06819_b200 import bang as b
+    b.lib()                                    # fails loudly if libbang.so is missing
+    return b
+
+
+def assert_maps(g, o, prec, what=""):
+    g = np.asarray(g, dtype=np.float64)
+    o = np.asarray(o, dtype=np.float64)
+    assert g.shape == o.shape
+    rtol = RTOL[prec]
+    worst = []
+    for q in range(4):
+        gq, oq = g[..., q, :, :], o[..., q, :, :]
+        den = np.abs(oq)
+        if q == 1:
+            den = np.maximum(den, 1e-3 * np.abs(oq).max(axis=(-2, -1), keepdims=True))
+        atol = 1e-30 if (prec == "fp32" and q == 0) else 0.0
+        bad = np.abs(gq - oq) > rtol * den + atol
+        worst.append(float(np.max(np.abs(gq - oq) / (den + atol + 1e-300))))
+        assert not bad.any(), f"{what} map {q}: {bad.sum()} pixels beyond {rtol:g}, worst {worst[-1]:.3e}"
+    return worst
+
+
+def first_order_bound(maps_o, data, err, mask):
+    """sum_p |z_p| |m_p| / e_p over used pixels (reading Q), per theta."""
+    z = np.abs((data - maps_o) / err) * np.abs(maps_o) / err
+    return (z * mask).sum(axis=(-3, -2, -1))
+
+
+def assert_logl(g, o, maps_o, data, err, mask, prec, near=None, what=""):
+    g, o = np.asarray(g), np.asarray(o)
+    bound = RTOL[prec] * first_order_bound(maps_o, data, err, mask) + 1e-9 * np.abs(o) * (prec == "fp32") + 1e-7
+    d = np.abs(g - o)
+    assert (d <= bound).all(), f"{what}: |dlogL| {d.max():.3e} beyond first-order bound (worst ratio {(d / bound).max():.3e})"
+    if near is not None and prec == "fp32" and near.any():
+        npix = mask[0].sum()
+        lim = 1e-3 * math.sqrt(npix)
+        assert (d[near] <= lim).all(), f"{what}: near-truth |dlogL| {d[near].max():.3e} > 1e-3 sqrt(N_pix) = {lim:.3e}"
+    return float(d.max())
+
+
+class Case:
+    """Seeded inputs + oracle results for one config (or one config-4 variant) on a parity subset of the batch."""
+
+    def __init__(self, oracle, idx, nsub, variant=None):
+        self.idx, self.variant = idx, variant
+        self.cfg = W.config(idx, variant)
+        richest = W.config(idx)                               # data come from the richest model (config 4)
+        self.theta = W.theta_batch(idx)
+        self.B = self.theta.shape[0]
+        self.sub = W.parity_subset(idx, self.B, nsub)
+        slots = W.near_truth_slots(idx, self.B)
+        self.near = np.isin(self.sub, slots) if (idx != 1 and variant in (None, "B+2D+H")) else np.zeros(len(self.sub), bool)
+        mtrue = oracle.model_maps(W.theta_true(idx), richest)[0]
+        self.data, self.err, self.mask = W.make_data(idx, mtrue)
+        self.logl_o, self.maps_o = oracle.loglike(self.theta[self.sub], self.cfg, self.data, self.err, self.mask,
+                                                  return_maps=True)
+
+
+_cases = {}
+
+
+def get_case(oracle, idx, nsub, variant=None):
+    key = (idx, variant)
+    if key not in _cases:
+        _cases[key] = Case(oracle, idx, nsub, variant)
+    return _cases[key]
+
+
+def run_case(bang, case, prec, full_batch):
+    import torch
+    ctx = bang.Context(case.cfg, precision=prec)
+    ctx.set_data(case.data, case.err, case.mask)
+    th_sub = case.theta[case.sub]
+    maps = ctx.model_maps(th_sub).cpu().numpy()
+    if full_batch:                                           # bench.py's launch configuration: the whole batch at once
+        ll_all = ctx.loglike(torch.as_tensor(case.theta, device="cuda")).cpu().numpy()
+        ll = ll_all[case.sub]
+    else:
+        ll_all = None
+        ll = ctx.loglike(th_sub).cpu().numpy()
+    ctx.close()
+    return maps, ll, ll_all
+
+
+# ------------------------------------------------------------------------------------------------ config 1
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_config1_tiny(bang, oracle, prec):
+    case = get_case(oracle, 1, 1)
+    ctx = bang.Context(case.cfg, precision=prec)
+    # intermediate of steps a0-a3: the un-convolved fine maps (Alg. 1 line 3)
+    fine = ctx.model_fine(case.theta[:1]).cpu().numpy()[0]
+    fine_o = oracle.model_fine(case.theta[0], case.cfg)
+    assert fine.shape == fine_o.shape == (4, 32 * 2 + 12, 32 * 2 + 12)
+    assert_maps(fine, fine_o, prec, "fine")
+    ctx.close()
+    maps, ll, _ = run_case(bang, case, prec, full_batch=False)
+    assert_maps(maps, case.maps_o, prec, "maps")
+    assert_logl(ll, case.logl_o, case.maps_o, case.data, case.err, case.mask, prec, near=np.array([True]), what="cfg1")
+
+
+def test_config1_matches_the_survey_crosscheck_pixels(bang):
+    # tests/golden/config1_survey_crosscheck.txt: an independent prototype's values
+    import os
+    ctx = bang.Context(W.config(1), precision="fp64")
+    m = ctx.model_maps(W.theta_true(1)).cpu().numpy()[0]
+    ctx.close()
+    path = os.path.join(os.path.dirname(__file__), "golden", "config1_survey_crosscheck.txt")
+    for line in open(path):
+        if line.startswith("#"):
+            continue
+        i, j, *vals = line.split()
+        for q, v in enumerate(vals):
+            assert abs(m[q, int(i), int(j)] / float(v) - 1) < 1e-9
+
+
+# ------------------------------------------------------------------------------------------------ configs 2, 3, 5
+@pytest.mark.parametrize("idx,nsub,prec", [(2, 32, "fp32"), (2, 32, "fp64"), (3, 20, "fp32"), (3, 20, "fp64"),
+                                           (5, 17, "fp32")])
+def test_config_batches_against_oracle(bang, oracle, idx, nsub, prec):
+    case = get_case(oracle, idx, nsub)
+    full = prec == "fp32" or idx == 2
+    maps, ll, ll_all = run_case(bang, case, prec, full_batch=full)
+    assert_maps(maps, case.maps_o, prec, f"cfg{idx}")
+    assert_logl(ll, case.logl_o, case.maps_o, case.data, case.err, case.mask, prec, near=case.near, what=f"cfg{idx}")
+    if ll_all is not None:
+        assert ll_all.shape == (case.B,) and np.isfinite(ll_all).all()
+
+
+# ------------------------------------------------------------------------------------------------ config 4
+@pytest.mark.parametrize("variant", ["B+D", "B+2D", "2D+H", "B+2D+H"])
+def test_config4_model_variants(bang, oracle, variant):
+    case = get_case(oracle, 4, 20, variant)
+    maps, ll, ll_all = run_case(bang, case, "fp32", full_batch=True)
+    assert_maps(maps, case.maps_o, "fp32", variant)
+    assert_logl(ll, case.logl_o, case.maps_o, case.data, case.err, case.mask, "fp32", near=case.near, what=variant)
+    assert np.isfinite(ll_all).all()
+    if variant == "B+2D+H":           # the model that generated the data explains it best near the truth
+        others = [get_case(oracle, 4, 20, v) for v in ("B+D", "2D+H")]
+        for o in others:
+            assert case.logl_o[case.near].max() > o.logl_o.max()
+
+
+# ------------------------------------------------------------------------------------------------ properties at full size
+@pytest.mark.parametrize("idx", [2, 3, 4, 5])
+def test_fp32_and_fp64_modes_agree_on_the_whole_batch(bang, oracle, idx):
+    import torch
+    case = get_case(oracle, idx, {2: 32, 3: 20, 4: 20, 5: 17}[idx], "B+2D+H" if idx == 4 else None)
+    B = case.B if idx != 5 else 1024
+    th = torch.as_tensor(case.theta[:B], device="cuda")
+    out = {}
+    for prec in ("fp32", "fp64"):
+        ctx = bang.Context(case.cfg, precision=prec)
+        ctx.set_data(case.data, case.err, case.mask)
+        out[prec] = ctx.loglike(th).cpu().numpy()
+        ctx.close()
+    assert np.isfinite(out["fp64"]).all()
+    rel = np.abs(out["fp32"] - out["fp64"]) / np.abs(out["fp64"])
+    assert rel.max() < 2e-5, rel.max()          # far from the truth logL ~ -1e8: a 1e-4 per-pixel tolerance allows ~2e-4
+
+
+def test_batch_results_do_not_depend_on_batch_size_or_order(bang, oracle):
+    import torch
+    case = get_case(oracle, 2, 32)
+    ctx = bang.Context(case.cfg, precision="fp32")
+    ctx.set_data(case.data, case.err, case.mask)
+    th = torch.as_tensor(case.theta, device="cuda")
+    a = ctx.loglike(th).cpu().numpy()
+    b = ctx.loglike(th).cpu().numpy()
+    assert np.array_equal(a, b)                                     # deterministic
+    perm = np.random.default_rng(0).permutation(case.B)
+    c = ctx.loglike(th[torch.as_tensor(perm, device="cuda")]).cpu().numpy()
+    assert np.array_equal(c, a[perm])                               # each theta independent of its neighbours
+    d = ctx.loglike(th[:37]).cpu().numpy()
+    assert np.array_equal(d, a[:37])
+    e = ctx.loglike_host(case.theta[:100])
+    assert np.array_equal(e, a[:100])                               # host-buffer entry point, same kernels
+    ctx.close()
+
+
+def test_logl_equals_likelihood_of_the_returned_maps(bang, oracle):
+    # eq. 18 on the library's own maps, evaluated by the oracle's step 11: ties bang_loglike to bang_model_maps
+    case = get_case(oracle, 3, 20)
+    ctx = bang.Context(case.cfg, precision="fp64")
+    ctx.set_data(case.data, case.err, case.mask)
+    th = case.theta[case.sub][:6]
+    maps = ctx.model_maps(th).cpu().numpy()
+    ll = ctx.loglike(th).cpu().numpy()
+    ctx.close()
+    for b in range(len(th)):
+        want = oracle.loglike_of_maps(maps[b], case.data, case.err, case.mask)
+        assert abs(ll[b] - want) <= 1e-12 * abs(want)
