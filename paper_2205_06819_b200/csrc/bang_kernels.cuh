@@ -243,29 +243,52 @@ BANG_D void build_vc_table(const ThetaC<T>& c, const GridC& g, const FitC& fit, 
     __syncthreads();
 }
 
-// a2 + a3: one fine cell (buffer coordinates jx, jy) -> B_tot, v_los, sigma_los, <L/M>   (eqs. 4-15, 19)
+// per-theta constants of the fine-cell model, copied from shared memory into registers once per theta so that the
+// per-cell code below touches shared memory only for its table look-up
 template <typename T>
-BANG_D void eval_cell(const ThetaC<T>& c, const unsigned comps, const PolyTab<T>& btab, const T* __restrict__ vtab,
-                      int jx, int jy, T& oB, T& oV, T& oS, T& oLM) {
+struct CellK {
+    int jcx, jcy, vfirst, vlast;
+    T hc, hs, xp0, yp0, inv_ci2;
+    T invRb2, ampBb, ampIb, MLb;
+    T cexp0, cexp1, ampBd0, ampBd1, MLd0, MLd1, vk0, vk1, q30, q31;
+};
+template <typename T>
+BANG_D CellK<T> load_cellk(const ThetaC<T>& c) {
+    CellK<T> k;
+    k.jcx = c.jcx; k.jcy = c.jcy; k.vfirst = c.vfirst; k.vlast = c.vcells - 1;
+    k.hc = c.hc; k.hs = c.hs; k.xp0 = c.xp0; k.yp0 = c.yp0; k.inv_ci2 = c.inv_ci2;
+    k.invRb2 = c.invRb2; k.ampBb = c.ampBb; k.ampIb = c.ampIb; k.MLb = c.MLb;
+    k.cexp0 = c.cexp[0]; k.cexp1 = c.cexp[1]; k.ampBd0 = c.ampBd[0]; k.ampBd1 = c.ampBd[1];
+    k.MLd0 = c.MLd[0]; k.MLd1 = c.MLd[1]; k.vk0 = c.vk[0]; k.vk1 = c.vk[1]; k.q30 = c.q3[0]; k.q31 = c.q3[1];
+    return k;
+}
+
+// a2 + a3: one fine cell, a = jx - jcx and b = jy - jcy (offsets in cells from the cell nearest to the galaxy centre)
+// -> B_tot, v_los, sigma_los, <L/M>   (eqs. 4-15, 19).  BULGE: the model has a bulge; SHIFT = 0/1/2/3: without a bulge
+// the disc exponentials are scaled by disc 1 (1), disc 2 (2) or the larger of the two (3) so that the ratios below
+// survive fp32 underflow far outside small discs.
+template <typename T, bool BULGE, int SHIFT>
+BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int bfirst, const int blast,
+                      const T* __restrict__ vtab, const int ai, const int bi, T& oB, T& oV, T& oS, T& oLM) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     // sec. 2.1: rotate into the galaxy frame (fn 2); R on the sky (bulge), r in the disc plane
-    const T a = (T)(jx - c.jcx), b = (T)(jy - c.jcy);
-    const T xp = fma(a, c.hc, fma(b, c.hs, c.xp0));
-    const T yp = fma(b, c.hc, fma(-a, c.hs, c.yp0));
+    const T a = (T)ai, b = (T)bi;
+    const T xp = fma(a, k.hc, fma(b, k.hs, k.xp0));
+    const T yp = fma(b, k.hc, fma(-a, k.hs, k.yp0));
     const T floor2 = sizeof(T) == 4 ? T(0x1p-32f) : T(0x1p-32);
     const T y2 = yp * yp;
-    const T R2 = fmax(fma(xp, xp, y2), floor2);
-    const T r2 = fmax(fma(xp, xp, y2 * c.inv_ci2), floor2);
+    const T r2 = fmax(fma(xp, xp, y2 * k.inv_ci2), floor2);
     const T rinv = fast_rsqrt(r2);
     const T r = r2 * rinv;
     const T cosphi = xp * rinv;
 
     // bulge: Sigma_b (eq. 4) and Sigma_b sigma_b^2 (eq. 6) from the scale-free tables at s^2 = R^2/R_b^2
     T Bb = T(0), IbL = T(0);
-    if (comps & C_BULGE) {
+    if constexpr (BULGE) {
+        const T R2 = fmax(fma(xp, xp, y2), floor2);
         T t;
-        const int cell = (int)min((unsigned)(tab_cell(R2 * c.invRb2, t) - btab.first), (unsigned)(btab.n_cells - 1));
-        const T* p = btab.coef + (size_t)cell * (2 * NC);
+        const int cell = (int)min((unsigned)(tab_cell(R2 * k.invRb2, t) - bfirst), (unsigned)blast);
+        const T* p = bcoef + (size_t)cell * (2 * NC);
         T cs[NC], cj[NC];
         if constexpr (sizeof(T) == 4) {
             const float4 v0 = __ldg(reinterpret_cast<const float4*>(p));
@@ -280,23 +303,20 @@ BANG_D void eval_cell(const ThetaC<T>& c, const unsigned comps, const PolyTab<T>
                 cs[d] = v0.x; cs[d + 1] = v0.y; cj[d] = v1.x; cj[d + 1] = v1.y;
             }
         }
-        Bb = c.ampBb * horner<T, D>(cs, t);
-        IbL = c.ampIb * horner<T, D>(cj, t);
+        Bb = k.ampBb * horner<T, D>(cs, t);
+        IbL = k.ampIb * horner<T, D>(cj, t);
     }
-    // discs: eq. 7-8.  Without a bulge the two exponentials are scaled by the larger one so that the ratios below
-    // survive fp32 underflow far outside small discs.
-    const T e1a = r * c.cexp[0], e2a = r * c.cexp[1];
+    // discs: eq. 7-8
+    const T e1a = r * k.cexp0, e2a = r * k.cexp1;
     T shift = T(0);
-    if (!(comps & C_BULGE)) {
-        shift = (comps & C_DISC1) ? ((comps & C_DISC2) ? fmax(e1a, e2a) : e1a) : e2a;
-    }
-    const T Bd1 = c.ampBd[0] * fast_exp2(e1a - shift);
-    const T Bd2 = c.ampBd[1] * fast_exp2(e2a - shift);
+    if constexpr (!BULGE) shift = SHIFT == 1 ? e1a : (SHIFT == 2 ? e2a : fmax(e1a, e2a));
+    const T Bd1 = k.ampBd0 * fast_exp2(e1a - shift);
+    const T Bd2 = k.ampBd1 * fast_exp2(e2a - shift);
     // v_c(r) from the per-theta table (eq. 10)
     T vc;
     {
         T t;
-        const int cell = (int)min((unsigned)(tab_cell(r2, t) - c.vfirst), (unsigned)(c.vcells - 1));
+        const int cell = (int)min((unsigned)(tab_cell(r2, t) - k.vfirst), (unsigned)k.vlast);
         const T* p = vtab + cell * NC;
         T cv[NC];
         if constexpr (sizeof(T) == 4) {
@@ -313,14 +333,45 @@ BANG_D void eval_cell(const ThetaC<T>& c, const unsigned comps, const PolyTab<T>
     }
     // eq. 13, 14 (with 11), 15 (with 12), 19
     const T Btot = Bb + Bd1 + Bd2;
-    const T Stot = fma(c.MLb, Bb, fma(c.MLd[0], Bd1, c.MLd[1] * Bd2));     // total mass surface density (x 1e-6)
+    const T Stot = fma(k.MLb, Bb, fma(k.MLd0, Bd1, k.MLd1 * Bd2));         // total mass surface density (x 1e-6)
     const T invB = fast_rcp(Btot);
-    const T kB = fma(c.vk[0], Bd1, c.vk[1] * Bd2);
-    const T qB = fma(c.q3[0], Bd1, c.q3[1] * Bd2);
+    const T kB = fma(k.vk0, Bd1, k.vk1 * Bd2);
+    const T qB = fma(k.q30, Bd1, k.q31 * Bd2);
     oV = cosphi * vc * kB * invB;
     oS = fast_sqrt(fma(vc * vc, qB, IbL) * invB);
     oLM = Btot * fast_rcp(Stot);
-    oB = (comps & C_BULGE) ? Btot : Btot * fast_exp2(shift);
+    oB = BULGE ? Btot : Btot * fast_exp2(shift);
+}
+
+// a2 + a3 over a run of whole fine rows: cells i = tid, tid + NT, ... of the n_rows x nfx block that starts at fine row
+// jy0, written to dst[row * row_pitch + observable * obs_stride + x].  All threads of the CTA take part.
+template <typename T, bool BULGE, int SHIFT>
+BANG_D void eval_rows(const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab, T* __restrict__ dst,
+                      const size_t row_pitch, const size_t obs_stride, const int nfx, const int jy0, const int n_rows,
+                      const int tid, const int NT) {
+    const int step_j = NT / nfx, step_x = NT - step_j * nfx;
+    int j = tid / nfx, x = tid - j * nfx;
+    const int n = n_rows * nfx;
+    const T* __restrict__ bcoef = btab.coef;
+    const int bfirst = btab.first, blast = btab.n_cells - 1;
+    for (int i = tid; i < n; i += NT) {
+        T vB, vV, vS, vL;
+        eval_cell<T, BULGE, SHIFT>(k, bcoef, bfirst, blast, vtab, x - k.jcx, jy0 + j - k.jcy, vB, vV, vS, vL);
+        T* d = dst + (size_t)j * row_pitch + x;
+        d[0] = vB; d[obs_stride] = vV; d[2 * obs_stride] = vS; d[3 * obs_stride] = vL;
+        x += step_x; j += step_j;
+        if (x >= nfx) { x -= nfx; ++j; }
+    }
+}
+template <typename T>
+BANG_D void eval_rows_any(const unsigned comps, const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab,
+                          T* __restrict__ dst, const size_t row_pitch, const size_t obs_stride, const int nfx,
+                          const int jy0, const int n_rows, const int tid, const int NT) {
+    if (comps & C_BULGE) eval_rows<T, true, 0>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, tid, NT);
+    else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
+        eval_rows<T, false, 3>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, tid, NT);
+    else if (comps & C_DISC1) eval_rows<T, false, 1>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, tid, NT);
+    else eval_rows<T, false, 2>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, tid, NT);
 }
 
 // ---- the fused kernel ---------------------------------------------------------------------------------------------
@@ -420,6 +471,7 @@ __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedPara
             continue;
         }
         build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
+        const CellK<T> k = load_cellk<T>(c);
 
         T acc[P][NACC];
 #pragma unroll
@@ -431,17 +483,10 @@ __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedPara
         for (int sr = 0; sr < nsuper; ++sr) {
             // ---- a2 + a3: evaluate the S fine rows of this super-row into shared memory
             {
-                int j = 0, x = tid;
-                while (x >= g.nfx) { x -= g.nfx; ++j; }
-                for (int i = tid; i < ncell_sr; i += NT) {
-                    const int jy = sr * S + j;
-                    T vB = T(0), vV = T(0), vS = T(0), vL = T(0);
-                    if (jy < g.nfy) eval_cell<T>(c, g.comps, p.btab, vtab, x, jy, vB, vV, vS, vL);
-                    T* dst = rowbuf + (size_t)(j * 4) * nfb + x;
-                    dst[0] = vB; dst[nfb] = vV; dst[2 * nfb] = vS; dst[3 * nfb] = vL;
-                    x += NT;
-                    while (x >= g.nfx) { x -= g.nfx; ++j; }
-                }
+                const int n_rows = min(S, max(g.nfy - sr * S, 0));
+                eval_rows_any<T>(g.comps, k, p.btab, vtab, rowbuf, (size_t)4 * nfb, (size_t)nfb, g.nfx, sr * S, n_rows, tid, NT);
+                if (n_rows < S)                       // rows past the grid (tap padding): their weights are zero, keep them finite
+                    for (int i = tid; i < (S - n_rows) * 4 * nfb; i += NT) rowbuf[(size_t)n_rows * 4 * nfb + i] = T(0);
             }
             __syncthreads();
             // ---- a4 + a5: PSF along x fused with the rebin, then scattered along y into the running data rows
@@ -533,12 +578,8 @@ __global__ void __launch_bounds__(256) k_fine(const __grid_constant__ FineParams
             continue;
         }
         build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
-        for (size_t i = threadIdx.x; i < plane; i += blockDim.x) {
-            const int jy = (int)(i / g.nfx), jx = (int)(i - (size_t)jy * g.nfx);
-            T vB, vV, vS, vL;
-            eval_cell<T>(c, g.comps, p.btab, vtab, jx, jy, vB, vV, vS, vL);
-            out[i] = vB; out[plane + i] = vV; out[2 * plane + i] = vS; out[3 * plane + i] = vL;
-        }
+        const CellK<T> k = load_cellk<T>(c);
+        eval_rows_any<T>(g.comps, k, p.btab, vtab, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy, threadIdx.x, blockDim.x);
     }
 }
 
