@@ -13,9 +13,9 @@
 namespace bang {
 namespace {
 
-template <typename T, int S, int NACC, int P>
-cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
-    auto kern = k_fused<T, S, NACC, P>;
+template <typename T, int S, int NACC, int P, int MODE>
+cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) {
+    auto kern = k_fused<T, S, NACC, P, MODE>;
     const size_t smem = fused_smem_bytes<T>(S, L.nfb);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -34,8 +34,8 @@ cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
     if (getenv("BANG_VERBOSE")) {
         cudaFuncAttributes fa;
         cudaFuncGetAttributes(&fa, kern);
-        fprintf(stderr, "[bang] k_fused<%s,S=%d,NACC=%d,P=%d> regs=%d smem=%zu threads=%d ctas/SM=%d grid=%d B=%d\n",
-                sizeof(T) == 4 ? "f32" : "f64", S, NACC, P, fa.numRegs, smem, L.threads, per_sm, ctas, L.B);
+        fprintf(stderr, "[bang] k_fused<%s,S=%d,NACC=%d,P=%d,MODE=%d> regs=%d smem=%zu threads=%d ctas/SM=%d grid=%d B=%d\n",
+                sizeof(T) == 4 ? "f32" : "f64", S, NACC, P, MODE, fa.numRegs, smem, L.threads, per_sm, ctas, L.B);
     }
 
     FusedParams<T, S, NACC> p;
@@ -43,10 +43,15 @@ cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
     p.btab = PolyTab<T>{static_cast<const T*>(L.btab), L.btab_first, L.btab_cells};
     p.Ftab = PolyTab<T>{static_cast<const T*>(L.Ftab), L.Ftab_first, L.Ftab_cells};
     for (int t = 0; t < NACC * S; ++t) p.W[t] = (T)L.W[t];
-    p.theta = L.theta; p.B = L.B; p.nxp = L.nxp; p.nfb = L.nfb; p.mode = L.mode;
+    p.theta = L.theta; p.B = L.B; p.nxp = L.nxp; p.nfb = L.nfb;
     p.maps = static_cast<T*>(L.maps); p.data = L.data; p.C0 = L.C0; p.logL = L.logL;
-    k_fused<T, S, NACC, P><<<ctas, L.threads, smem, L.stream>>>(p);
+    kern<<<ctas, L.threads, smem, L.stream>>>(p);
     return cudaGetLastError();
+}
+
+template <typename T, int S, int NACC, int P>
+cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
+    return L.mode == 0 ? launch_mode<T, S, NACC, P, 0>(L, info, query_only) : launch_mode<T, S, NACC, P, 1>(L, info, query_only);
 }
 
 template <typename T, int S, int P>

@@ -345,12 +345,20 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int 
 
 // a2 + a3 over a run of whole fine rows: cells i = tid, tid + NT, ... of the n_rows x nfx block that starts at fine row
 // jy0, written to dst[row * row_pitch + observable * obs_stride + x].  All threads of the CTA take part.
+struct EvalWalk { int i0, j0, x0, step_j, step_x; };   // flat cell i = i0 + n NT sits at (row j, column x)
+BANG_D EvalWalk make_walk(const int tid, const int NT, const int nfx) {
+    EvalWalk w;
+    w.i0 = tid; w.j0 = tid / nfx; w.x0 = tid - w.j0 * nfx;
+    w.step_j = NT / nfx; w.step_x = NT - w.step_j * nfx;
+    return w;
+}
 template <typename T, bool BULGE, int SHIFT>
 BANG_D void eval_rows(const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab, T* __restrict__ dst,
                       const size_t row_pitch, const size_t obs_stride, const int nfx, const int jy0, const int n_rows,
-                      const int tid, const int NT) {
-    const int step_j = NT / nfx, step_x = NT - step_j * nfx;
-    int j = tid / nfx, x = tid - j * nfx;
+                      const EvalWalk& w, const int NT) {
+    const int step_j = w.step_j, step_x = w.step_x;
+    int j = w.j0, x = w.x0;
+    const int tid = w.i0;
     const int n = n_rows * nfx;
     const T* __restrict__ bcoef = btab.coef;
     const int bfirst = btab.first, blast = btab.n_cells - 1;
@@ -366,12 +374,12 @@ BANG_D void eval_rows(const CellK<T>& k, const PolyTab<T>& btab, const T* __rest
 template <typename T>
 BANG_D void eval_rows_any(const unsigned comps, const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab,
                           T* __restrict__ dst, const size_t row_pitch, const size_t obs_stride, const int nfx,
-                          const int jy0, const int n_rows, const int tid, const int NT) {
-    if (comps & C_BULGE) eval_rows<T, true, 0>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, tid, NT);
+                          const int jy0, const int n_rows, const EvalWalk& w, const int NT) {
+    if (comps & C_BULGE) eval_rows<T, true, 0>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_rows<T, false, 3>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, tid, NT);
-    else if (comps & C_DISC1) eval_rows<T, false, 1>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, tid, NT);
-    else eval_rows<T, false, 2>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, tid, NT);
+        eval_rows<T, false, 3>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else if (comps & C_DISC1) eval_rows<T, false, 1>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else eval_rows<T, false, 2>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
 }
 
 // ---- the fused kernel ---------------------------------------------------------------------------------------------
@@ -385,7 +393,6 @@ struct FusedParams {
     int B;
     int nxp;                     // data columns padded to a multiple of P
     int nfb;                     // row-buffer width in cells (>= (nxp-1+NACC) S, multiple of 4, plus over-read slack)
-    int mode;                    // 0: write maps, 1: reduce the likelihood
     T* maps;                     // [B][4][ny][nx]
     const double2* data;         // [ny][4][nxp] {d, 1/e} (1/e = 0 where masked or padded)
     double C0;                   // sum over used pixels of -1/2 ln(2 pi e^2)
@@ -432,7 +439,12 @@ BANG_D void load_run(const T* __restrict__ src, T (&f)[N]) {
     }
 }
 
-template <typename T, int S, int NACC, int P>
+// 1/x for the final M/L = 1/<L/M> (fn 10): MUFU.RCP (1 ulp) in fp32 mode, IEEE division in fp64 mode
+BANG_D float inv_ml(float x) { return fast_rcp(x); }
+BANG_D double inv_ml(double x) { return 1.0 / x; }
+
+// MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike)
+template <typename T, int S, int NACC, int P, int MODE>
 __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     constexpr int RUN = (P - 1 + NACC) * S;          // fine cells one thread reads per row for its P data pixels
@@ -451,9 +463,12 @@ __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedPara
     const int G = p.nxp / P;                         // pixel groups per map
     const int items = 4 * G;
     const int q = tid / G, grp = tid - q * G;        // this thread's observable and pixel group in the PSF phase
+    const bool psf_thread = tid < items;
     const int nsuper = g.ny + NACC - 1;
-    const int ncell_sr = S * g.nfx;                  // cells evaluated per super-row
     const size_t npix = (size_t)g.nx * g.ny;
+    // the walk of this thread over the S x nfx cells of a super-row (a2 + a3): start (row, column) and stride
+    const EvalWalk walk = make_walk(tid, NT, g.nfx);
+    const T* run_base = rowbuf + (size_t)q * nfb + grp * (P * S);
 
     for (int i = tid; i < S * 4 * nfb; i += NT) rowbuf[i] = T(0);
 
@@ -462,7 +477,7 @@ __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedPara
         if (tid == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, c);
         __syncthreads();
         if (!c.valid) {                              // out-of-domain theta: NaN maps / -inf likelihood
-            if (p.mode == 0) {
+            if constexpr (MODE == 0) {
                 const T qnan = (T)nan("");
                 for (size_t i = tid; i < 4 * npix; i += NT) p.maps[(size_t)b * 4 * npix + i] = qnan;
             } else if (tid == 0) {
@@ -477,70 +492,77 @@ __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedPara
 #pragma unroll
         for (int i = 0; i < P; ++i)
 #pragma unroll
-            for (int k = 0; k < NACC; ++k) acc[i][k] = T(0);
+            for (int kk = 0; kk < NACC; ++kk) acc[i][kk] = T(0);
         double chi2 = 0.0;
 
         for (int sr = 0; sr < nsuper; ++sr) {
             // ---- a2 + a3: evaluate the S fine rows of this super-row into shared memory
             {
                 const int n_rows = min(S, max(g.nfy - sr * S, 0));
-                eval_rows_any<T>(g.comps, k, p.btab, vtab, rowbuf, (size_t)4 * nfb, (size_t)nfb, g.nfx, sr * S, n_rows, tid, NT);
+                eval_rows_any<T>(g.comps, k, p.btab, vtab, rowbuf, (size_t)4 * nfb, (size_t)nfb, g.nfx, sr * S, n_rows, walk, NT);
                 if (n_rows < S)                       // rows past the grid (tap padding): their weights are zero, keep them finite
                     for (int i = tid; i < (S - n_rows) * 4 * nfb; i += NT) rowbuf[(size_t)n_rows * 4 * nfb + i] = T(0);
             }
             __syncthreads();
             // ---- a4 + a5: PSF along x fused with the rebin, then scattered along y into the running data rows
-            if (tid < items) {
+            if (psf_thread) {
+                const int py = sr - (NACC - 1);      // the data row this super-row completes
+                // a6: this thread's P {d, 1/e} pairs, requested now and used after the taps (the row is padded to nxp,
+                // so the loads need no guard; 1/e = 0 where masked or padded)
+                double2 de[P];
+                if constexpr (MODE == 1) {
+                    if (py >= 0) {
+                        const double2* src = p.data + ((size_t)py * 4 + q) * p.nxp + grp * P;
+#pragma unroll
+                        for (int i = 0; i < P; ++i) de[i] = __ldg(src + i);
+                    }
+                }
 #pragma unroll
                 for (int j = 0; j < S; ++j) {
                     T f[RUN];
-                    load_run<T, RUN, ALIGN>(rowbuf + (size_t)(j * 4 + q) * nfb + grp * (P * S), f);
+                    load_run<T, RUN, ALIGN>(run_base + (size_t)(j * 4) * nfb, f);
 #pragma unroll
                     for (int i = 0; i < P; ++i) {
                         T xp = T(0);
 #pragma unroll
                         for (int t = 0; t < NACC * S; ++t) xp = fma(p.W[t], f[i * S + t], xp);
 #pragma unroll
-                        for (int k = 0; k < NACC; ++k) acc[i][k] = fma(p.W[(NACC - 1 - k) * S + j], xp, acc[i][k]);
+                        for (int kk = 0; kk < NACC; ++kk) acc[i][kk] = fma(p.W[(NACC - 1 - kk) * S + j], xp, acc[i][kk]);
                     }
                 }
                 // ---- a6 (or map output): data row py is complete
-                const int py = sr - (NACC - 1);
                 if (py >= 0) {
 #pragma unroll
                     for (int i = 0; i < P; ++i) {
                         const int px = grp * P + i;
                         T m = acc[i][0];
-                        if (q == 3) m = T(1) / m;                      // M/L = 1/<L/M> (fn 10)
-                        if (px < g.nx) {
-                            if (p.mode == 0) {
-                                p.maps[((size_t)b * 4 + q) * npix + (size_t)py * g.nx + px] = m;
-                            } else {
-                                const double2 de = __ldg(p.data + ((size_t)py * 4 + q) * p.nxp + px);
-                                const double z = (de.x - (double)m) * de.y;   // eq. 18, residual in fp64
-                                chi2 = fma(z, z, chi2);
-                            }
+                        if (q == 3) m = inv_ml(m);                     // M/L = 1/<L/M> (fn 10)
+                        if constexpr (MODE == 0) {
+                            if (px < g.nx) p.maps[((size_t)b * 4 + q) * npix + (size_t)py * g.nx + px] = m;
+                        } else {
+                            const double z = (de[i].x - (double)m) * de[i].y;      // eq. 18, residual in fp64
+                            chi2 = (px < g.nx) ? fma(z, z, chi2) : chi2;
                         }
                     }
                 }
 #pragma unroll
                 for (int i = 0; i < P; ++i) {
 #pragma unroll
-                    for (int k = 0; k + 1 < NACC; ++k) acc[i][k] = acc[i][k + 1];
+                    for (int kk = 0; kk + 1 < NACC; ++kk) acc[i][kk] = acc[i][kk + 1];
                     acc[i][NACC - 1] = T(0);
                 }
             }
             __syncthreads();
         }
-        if (p.mode == 1) {                           // a6: block reduction, warp shuffles, fp64
+        if constexpr (MODE == 1) {                   // a6: block reduction, warp shuffles, fp64
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) chi2 += __shfl_xor_sync(0xffffffffu, chi2, o);
             if ((tid & 31) == 0) red[tid >> 5] = chi2;
             __syncthreads();
             if (tid == 0) {
-                double s = 0.0;
-                for (int w = 0; w < (NT + 31) / 32; ++w) s += red[w];
-                p.logL[b] = p.C0 - 0.5 * s;
+                double sum = 0.0;
+                for (int w = 0; w < (NT + 31) / 32; ++w) sum += red[w];
+                p.logL[b] = p.C0 - 0.5 * sum;
             }
         }
     }
@@ -579,7 +601,8 @@ __global__ void __launch_bounds__(256) k_fine(const __grid_constant__ FineParams
         }
         build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
         const CellK<T> k = load_cellk<T>(c);
-        eval_rows_any<T>(g.comps, k, p.btab, vtab, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy, threadIdx.x, blockDim.x);
+        eval_rows_any<T>(g.comps, k, p.btab, vtab, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy,
+                         make_walk(threadIdx.x, blockDim.x, g.nfx), blockDim.x);
     }
 }
 
