@@ -239,10 +239,13 @@ def run_ours(args):
     clocks = clk.summary()
     assert torch.isfinite(out).all()
 
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic = None                                             # DRAM bytes per k_fused launch from the ncu capture
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(workload_name(idx, prec))
+        import csv
+        for row in csv.DictReader(open(tp)):
+            if row["workload"] == workload_name(idx, prec):
+                traffic = float(row["dram_bytes_per_launch"])
     roof = R.roofline(B * ncell, statistics.mean(times), cfg["supersample"], rk, prec, clocks.get("sm_mhz"), traffic)
     roof["kernel"] = "k_fused"
     roof["kernel_ms_best"] = 1e3 * min(times)
