@@ -38,7 +38,7 @@ def _units():
 def _compile(unit):
     obj, src, defs = unit
     out = os.path.join(OBJ, obj)
-    cmd = [NVCC, *FLAGS, *defs, "-c", src, "-o", out]
+    cmd = [NVCC, *FLAGS, *os.environ.get("BANG_NVCC_EXTRA", "").split(), *defs, "-c", src, "-o", out]
     r = subprocess.run(cmd, capture_output=True, text=True)
     with open(out + ".log", "w") as f:
         f.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)

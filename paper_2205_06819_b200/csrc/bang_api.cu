@@ -139,9 +139,9 @@ __global__ void k_univ_fit(int n_rows, FitC fit, const double* __restrict__ vals
     }
 }
 
-// data preparation: {d, 1/e} per used pixel ({0,0} where masked or padded), C0 = sum -1/2 ln(2 pi e^2), and the number
+// data preparation (layout [ny][4][P][nxp/P]): {d, 1/e} per used pixel ({0,0} where masked or padded), C0 = sum -1/2 ln(2 pi e^2), and the number
 // of used pixels with err <= 0 or a non-finite value.  One block, deterministic reduction order.
-__global__ void k_prep_data(int nx, int ny, int nxp, const double* __restrict__ data, const double* __restrict__ err,
+__global__ void k_prep_data(int nx, int ny, int nxp, int P, const double* __restrict__ data, const double* __restrict__ err,
                             const unsigned char* __restrict__ mask, double2* __restrict__ out, double* __restrict__ scal) {
     __shared__ double sh[2][32];
     double c0 = 0.0, bad = 0.0;
@@ -160,7 +160,8 @@ __global__ void k_prep_data(int nx, int ny, int nxp, const double* __restrict__ 
                 }
             }
         }
-        out[i] = v;
+        // [py][q][i][group]: pixel px = group P + i, so that the fused kernel's load of its i-th pixel is coalesced
+        out[(((size_t)py * 4 + q) * P + px % P) * (nxp / P) + px / P] = v;
     }
     for (int o = 16; o > 0; o >>= 1) {
         c0 += __shfl_xor_sync(0xffffffffu, c0, o);
@@ -398,7 +399,7 @@ int bang_set_data(bang_ctx* ctx, const double* data_dev, const double* err_dev, 
     double2* buf = nullptr;
     const size_t n = (size_t)ctx->g.ny * 4 * ctx->nxp;
     CU(cudaMalloc(&buf, n * sizeof(double2)));
-    k_prep_data<<<1, 1024, 0, ctx->stream>>>(ctx->g.nx, ctx->g.ny, ctx->nxp, data_dev, err_dev, mask_dev, buf, ctx->scal);
+    k_prep_data<<<1, 1024, 0, ctx->stream>>>(ctx->g.nx, ctx->g.ny, ctx->nxp, ctx->P, data_dev, err_dev, mask_dev, buf, ctx->scal);
     ctx->launches += 1;
     double scal[2] = {0, 0};
     cudaError_t e = cudaGetLastError();

@@ -13,9 +13,10 @@
 namespace bang {
 namespace {
 
-template <typename T, int S, int NACC, int P, int MODE>
+template <typename T, int S, int NACC, int P, int MODE, int LBC>
 cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) {
-    auto kern = k_fused<T, S, NACC, P, MODE>;
+    auto kern = k_fused<T, S, NACC, P, MODE, LBC>;
+    if (L.threads > lbc_threads(LBC)) return cudaErrorInvalidValue;
     const size_t smem = fused_smem_bytes<T>(S, L.nfb);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -34,8 +35,8 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     if (getenv("BANG_VERBOSE")) {
         cudaFuncAttributes fa;
         cudaFuncGetAttributes(&fa, kern);
-        fprintf(stderr, "[bang] k_fused<%s,S=%d,NACC=%d,P=%d,MODE=%d> regs=%d smem=%zu threads=%d ctas/SM=%d grid=%d B=%d\n",
-                sizeof(T) == 4 ? "f32" : "f64", S, NACC, P, MODE, fa.numRegs, smem, L.threads, per_sm, ctas, L.B);
+        fprintf(stderr, "[bang] k_fused<%s,S=%d,NACC=%d,P=%d,MODE=%d,LBC=%d> regs=%d smem=%zu threads=%d ctas/SM=%d grid=%d B=%d\n",
+                sizeof(T) == 4 ? "f32" : "f64", S, NACC, P, MODE, LBC, fa.numRegs, smem, L.threads, per_sm, ctas, L.B);
     }
 
     FusedParams<T, S, NACC> p;
@@ -49,9 +50,18 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     return cudaGetLastError();
 }
 
+template <typename T, int S, int NACC, int P, int LBC>
+cudaError_t launch_lbc(const FusedLaunch& L, FusedInfo* info, bool query_only) {
+    return L.mode == 0 ? launch_mode<T, S, NACC, P, 0, LBC>(L, info, query_only)
+                       : launch_mode<T, S, NACC, P, 1, LBC>(L, info, query_only);
+}
 template <typename T, int S, int NACC, int P>
 cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
-    return L.mode == 0 ? launch_mode<T, S, NACC, P, 0>(L, info, query_only) : launch_mode<T, S, NACC, P, 1>(L, info, query_only);
+    if constexpr (sizeof(T) == 4) {
+        if (L.threads <= 128) return launch_lbc<T, S, NACC, P, 0>(L, info, query_only);
+        if (L.threads <= 256) return launch_lbc<T, S, NACC, P, 1>(L, info, query_only);
+    }
+    return launch_lbc<T, S, NACC, P, 2>(L, info, query_only);
 }
 
 template <typename T, int S, int P>

@@ -263,18 +263,22 @@ BANG_D CellK<T> load_cellk(const ThetaC<T>& c) {
     return k;
 }
 
-// a2 + a3: one fine cell, a = jx - jcx and b = jy - jcy (offsets in cells from the cell nearest to the galaxy centre)
-// -> B_tot, v_los, sigma_los, <L/M>   (eqs. 4-15, 19).  BULGE: the model has a bulge; SHIFT = 0/1/2/3: without a bulge
+// sec. 2.1: rotate into the galaxy frame (fn 2).  a = jx - jcx and b = jy - jcy are offsets in cells from
+// the cell nearest to the galaxy centre, so that fp32 keeps relative precision in R near the centre.
+template <typename T>
+BANG_D void rotate_cell(const CellK<T>& k, const T a, const T b, T& xp, T& yp) {
+    xp = fma(a, k.hc, fma(b, k.hs, k.xp0));
+    yp = fma(b, k.hc, fma(-a, k.hs, k.yp0));
+}
+
+// a2 + a3: one fine cell at (xp, yp) in the galaxy frame -> B_tot, v_los, sigma_los, <L/M>   (eqs. 4-15, 19).  BULGE: the model has a bulge; SHIFT = 0/1/2/3: without a bulge
 // the disc exponentials are scaled by disc 1 (1), disc 2 (2) or the larger of the two (3) so that the ratios below
 // survive fp32 underflow far outside small discs.
 template <typename T, bool BULGE, int SHIFT>
 BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int bfirst, const int blast,
-                      const T* __restrict__ vtab, const int ai, const int bi, T& oB, T& oV, T& oS, T& oLM) {
+                      const T* __restrict__ vtab, const T xp, const T yp, T& oB, T& oV, T& oS, T& oLM) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
-    // sec. 2.1: rotate into the galaxy frame (fn 2); R on the sky (bulge), r in the disc plane
-    const T a = (T)ai, b = (T)bi;
-    const T xp = fma(a, k.hc, fma(b, k.hs, k.xp0));
-    const T yp = fma(b, k.hc, fma(-a, k.hs, k.yp0));
+    // (xp, yp): the cell in the galaxy frame; R on the sky (bulge), r in the disc plane
     const T floor2 = sizeof(T) == 4 ? T(0x1p-32f) : T(0x1p-32);
     const T y2 = yp * yp;
     const T r2 = fmax(fma(xp, xp, y2 * k.inv_ci2), floor2);
@@ -363,8 +367,9 @@ BANG_D void eval_rows(const CellK<T>& k, const PolyTab<T>& btab, const T* __rest
     const T* __restrict__ bcoef = btab.coef;
     const int bfirst = btab.first, blast = btab.n_cells - 1;
     for (int i = tid; i < n; i += NT) {
-        T vB, vV, vS, vL;
-        eval_cell<T, BULGE, SHIFT>(k, bcoef, bfirst, blast, vtab, x - k.jcx, jy0 + j - k.jcy, vB, vV, vS, vL);
+        T vB, vV, vS, vL, xp, yp;
+        rotate_cell<T>(k, (T)(x - k.jcx), (T)(jy0 + j - k.jcy), xp, yp);
+        eval_cell<T, BULGE, SHIFT>(k, bcoef, bfirst, blast, vtab, xp, yp, vB, vV, vS, vL);
         T* d = dst + (size_t)j * row_pitch + x;
         d[0] = vB; d[obs_stride] = vV; d[2 * obs_stride] = vS; d[3 * obs_stride] = vL;
         x += step_x; j += step_j;
@@ -382,6 +387,46 @@ BANG_D void eval_rows_any(const unsigned comps, const CellK<T>& k, const PolyTab
     else eval_rows<T, false, 2>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
 }
 
+// a2 + a3 for one super-row of the fused kernel (S fine rows jy0 .. jy0+S-1 = one data row): thread `vt` takes the fine
+// columns x = vt, vt + NT, ... and evaluates the S cells of each column in one iteration, so that the index arithmetic,
+// the rotation and the store address are shared by S cells and S independent dependency chains are in flight.
+// dst[(row * 4 + observable) * nfb + x].  GUARD: some of the S rows lie past the grid (zero-weight tap padding): they are
+// written as zeros.
+template <typename T, int S, bool BULGE, int SHIFT, bool GUARD>
+BANG_D void eval_superrow(const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab, T* __restrict__ dst,
+                          const int nfb, const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
+    const T* __restrict__ bcoef = btab.coef;
+    const int bfirst = btab.first, blast = btab.n_cells - 1;
+    const T b0 = (T)(jy0 - k.jcy);
+    const T bx = fma(b0, k.hs, k.xp0), by = fma(b0, k.hc, k.yp0);
+    for (int x = vt; x < nfx; x += NT) {
+        const T a = (T)(x - k.jcx);
+        const T px = fma(a, k.hc, bx), py = fma(-a, k.hs, by);
+        T* d = dst + x;
+#pragma unroll
+        for (int j = 0; j < S; ++j) {
+            T vB, vV, vS, vL;
+            if (GUARD && jy0 + j >= nfy) {
+                vB = vV = vS = vL = T(0);
+            } else {
+                const T xp = j == 0 ? px : fma((T)j, k.hs, px), yp = j == 0 ? py : fma((T)j, k.hc, py);
+                eval_cell<T, BULGE, SHIFT>(k, bcoef, bfirst, blast, vtab, xp, yp, vB, vV, vS, vL);
+            }
+            d[(j * 4 + 0) * nfb] = vB; d[(j * 4 + 1) * nfb] = vV; d[(j * 4 + 2) * nfb] = vS; d[(j * 4 + 3) * nfb] = vL;
+        }
+    }
+}
+template <typename T, int S, bool GUARD>
+BANG_D void eval_superrow_any(const unsigned comps, const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab,
+                              T* __restrict__ dst, const int nfb, const int nfx, const int nfy, const int jy0,
+                              const int vt, const int NT) {
+    if (comps & C_BULGE) eval_superrow<T, S, true, 0, GUARD>(k, btab, vtab, dst, nfb, nfx, nfy, jy0, vt, NT);
+    else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
+        eval_superrow<T, S, false, 3, GUARD>(k, btab, vtab, dst, nfb, nfx, nfy, jy0, vt, NT);
+    else if (comps & C_DISC1) eval_superrow<T, S, false, 1, GUARD>(k, btab, vtab, dst, nfb, nfx, nfy, jy0, vt, NT);
+    else eval_superrow<T, S, false, 2, GUARD>(k, btab, vtab, dst, nfb, nfx, nfy, jy0, vt, NT);
+}
+
 // ---- the fused kernel ---------------------------------------------------------------------------------------------
 template <typename T, int S, int NACC>
 struct FusedParams {
@@ -394,7 +439,7 @@ struct FusedParams {
     int nxp;                     // data columns padded to a multiple of P
     int nfb;                     // row-buffer width in cells (>= (nxp-1+NACC) S, multiple of 4, plus over-read slack)
     T* maps;                     // [B][4][ny][nx]
-    const double2* data;         // [ny][4][nxp] {d, 1/e} (1/e = 0 where masked or padded)
+    const double2* data;         // [ny][4][P][nxp/P] {d, 1/e} of pixel group P + i (1/e = 0 where masked or padded)
     double C0;                   // sum over used pixels of -1/2 ln(2 pi e^2)
     double* logL;                // [B]
 };
@@ -444,8 +489,16 @@ BANG_D float inv_ml(float x) { return fast_rcp(x); }
 BANG_D double inv_ml(double x) { return 1.0 / x; }
 
 // MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike)
-template <typename T, int S, int NACC, int P, int MODE>
-__global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
+// LBC: launch-bound class = the CTA-size bracket the kernel is compiled for, which fixes its register budget:
+//   0: <= 128 threads, 7 (P = 2) or 5 (P = 4) CTAs per SM;  1: <= 256 threads, 3 or 2 CTAs per SM;  2: <= 512 threads.
+// fp64 mode is compiled for class 2 only.
+#ifndef BANG_B1P4
+#define BANG_B1P4 2
+#endif
+constexpr int lbc_threads(int lbc) { return lbc == 0 ? 128 : (lbc == 1 ? 256 : 512); }
+constexpr int lbc_blocks(int lbc, int P) { return lbc == 0 ? (P == 2 ? 7 : 5) : (lbc == 1 ? (P == 2 ? 3 : BANG_B1P4) : 1); }
+template <typename T, int S, int NACC, int P, int MODE, int LBC>
+__global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P)) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     constexpr int RUN = (P - 1 + NACC) * S;          // fine cells one thread reads per row for its P data pixels
     constexpr int RUN_BYTES = P * S * (int)sizeof(T);   // byte stride between the runs of neighbouring threads
@@ -466,8 +519,6 @@ __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedPara
     const bool psf_thread = tid < items;
     const int nsuper = g.ny + NACC - 1;
     const size_t npix = (size_t)g.nx * g.ny;
-    // the walk of this thread over the S x nfx cells of a super-row (a2 + a3): start (row, column) and stride
-    const EvalWalk walk = make_walk(tid, NT, g.nfx);
     const T* run_base = rowbuf + (size_t)q * nfb + grp * (P * S);
 
     for (int i = tid; i < S * 4 * nfb; i += NT) rowbuf[i] = T(0);
@@ -486,7 +537,6 @@ __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedPara
             continue;
         }
         build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
-        const CellK<T> k = load_cellk<T>(c);
 
         T acc[P][NACC];
 #pragma unroll
@@ -494,15 +544,17 @@ __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedPara
 #pragma unroll
             for (int kk = 0; kk < NACC; ++kk) acc[i][kk] = T(0);
         double chi2 = 0.0;
+        int vt = (tid + 32 * (b & 3)) % NT;              // this thread's first fine column in the model phase (a2 + a3)
 
         for (int sr = 0; sr < nsuper; ++sr) {
             // ---- a2 + a3: evaluate the S fine rows of this super-row into shared memory
-            {
-                const int n_rows = min(S, max(g.nfy - sr * S, 0));
-                eval_rows_any<T>(g.comps, k, p.btab, vtab, rowbuf, (size_t)4 * nfb, (size_t)nfb, g.nfx, sr * S, n_rows, walk, NT);
-                if (n_rows < S)                       // rows past the grid (tap padding): their weights are zero, keep them finite
-                    for (int i = tid; i < (S - n_rows) * 4 * nfb; i += NT) rowbuf[(size_t)n_rows * 4 * nfb + i] = T(0);
-            }
+            // the per-theta constants are re-read from shared memory for every super-row (a handful of broadcast loads)
+            // so that they do not occupy registers during the PSF phase
+            const CellK<T> k = load_cellk<T>(c);
+            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, false>(g.comps, k, p.btab, vtab, rowbuf, nfb, g.nfx, g.nfy, sr * S, vt, NT);
+            else eval_superrow_any<T, S, true>(g.comps, k, p.btab, vtab, rowbuf, nfb, g.nfx, g.nfy, sr * S, vt, NT);
+            vt = vt + 32 < NT ? vt + 32 : vt + 32 - NT;      // rotate the column ownership by one warp: the ragged last
+                                                             // pass then falls on a different warp (scheduler) each time
             __syncthreads();
             // ---- a4 + a5: PSF along x fused with the rebin, then scattered along y into the running data rows
             if (psf_thread) {
@@ -512,9 +564,9 @@ __global__ void __launch_bounds__(512) k_fused(const __grid_constant__ FusedPara
                 double2 de[P];
                 if constexpr (MODE == 1) {
                     if (py >= 0) {
-                        const double2* src = p.data + ((size_t)py * 4 + q) * p.nxp + grp * P;
+                        const double2* src = p.data + ((size_t)py * 4 + q) * p.nxp + grp;
 #pragma unroll
-                        for (int i = 0; i < P; ++i) de[i] = __ldg(src + i);
+                        for (int i = 0; i < P; ++i) de[i] = __ldg(src + i * G);
                     }
                 }
 #pragma unroll

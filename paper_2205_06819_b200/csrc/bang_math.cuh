@@ -238,7 +238,8 @@ template <> struct TabCfg<double> { static constexpr int D = 7, M = 3; };
 BANG_HD int tab_cell(float u, float& t) {
 #if defined(__CUDA_ARCH__)
     const int bits = __float_as_int(u);
-    t = __int_as_float(((bits & 0x7FFFF) << 4) | 0x40000000) - 3.0f;
+    // tau = 1 + (low 19 mantissa bits) 2^-23 in [1, 1 + 2^-4);  t = 32 tau - 33, exact: one LOP3 and one FFMA
+    t = fmaf(__int_as_float((bits & 0x7FFFF) | 0x3F800000), 32.0f, -33.0f);
 #else
     union { float f; int i; } c; c.f = u;
     const int bits = c.i;
