@@ -123,7 +123,7 @@ class OracleLeg:
         assert np.isfinite(ll).all()
         return dt
 
-    def sample(self, budget_s, offset=0, max_n=64):
+    def sample(self, budget_s, offset=0, max_n=4096):
         n = int(max(1, min(max_n, budget_s / max(self.t1, 1e-3))))
         B = self.theta.shape[0]
         sub = (offset + np.arange(n)) % B

@@ -21,7 +21,7 @@ struct bang_ctx {
     int n_sm = 0;
     GridC g{};
     FitC fit{};
-    int rk = 0, nacc = 0, P = 0, nxp = 0, nfb = 0, threads = 0;
+    int rk = 0, nacc = 0, P = 0, nxp = 0, threads = 0;
     std::vector<double> W;                 // composite taps, nacc * s
     void* btab = nullptr; int btab_first = 0, btab_cells = 0;
     void* Ftab = nullptr; int Ftab_first = 0, Ftab_cells = 0;
@@ -221,7 +221,7 @@ FusedLaunch make_launch(const bang_ctx* c, const double* theta, int B, int mode,
     L.btab = c->btab; L.btab_first = c->btab_first; L.btab_cells = c->btab_cells;
     L.Ftab = c->Ftab; L.Ftab_first = c->Ftab_first; L.Ftab_cells = c->Ftab_cells;
     L.W = c->W.data(); L.nacc = c->nacc;
-    L.theta = theta; L.B = B; L.P = c->P; L.nxp = c->nxp; L.nfb = c->nfb; L.mode = mode;
+    L.theta = theta; L.B = B; L.P = c->P; L.nxp = c->nxp; L.mode = mode;
     L.maps = maps; L.data = c->data; L.C0 = c->C0; L.logL = logL;
     L.threads = c->threads; L.ctas = c->force_ctas; L.n_sm = c->n_sm; L.stream = c->stream;
     return L;
@@ -352,7 +352,7 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
 
     // launch shape: P data pixels per thread in the PSF phase, one thread per (observable, pixel group)
     const char* envP = getenv("BANG_P");
-    int P = f64 ? 2 : (grid->nx >= 96 ? 4 : 2);
+    int P = f64 ? 2 : (grid->nx > 64 ? 4 : 2);        // measured: P = 4 wins from 80 columns on even with idle PSF threads
     if (envP && !f64 && (atoi(envP) == 2 || atoi(envP) == 4)) P = atoi(envP);
     ctx->P = P;
     ctx->nxp = (grid->nx + P - 1) / P * P;
@@ -362,7 +362,6 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     if (envT && atoi(envT) >= ctx->threads && atoi(envT) <= 512) ctx->threads = atoi(envT) / 32 * 32;
     const char* envC = getenv("BANG_CTAS");
     if (envC && atoi(envC) > 0) ctx->force_ctas = atoi(envC);
-    ctx->nfb = ((ctx->nxp - 1 + nacc) * s + 3) / 4 * 4 + 4;
     if (ctx->threads > 512) { delete ctx; return BANG_EINVAL; }      // row too wide for one CTA
     make_fit(f64 ? TabCfg<double>::D : TabCfg<float>::D, ctx->fit);
 

@@ -17,7 +17,7 @@ template <typename T, int S, int NACC, int P, int MODE, int LBC>
 cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) {
     auto kern = k_fused<T, S, NACC, P, MODE, LBC>;
     if (L.threads > lbc_threads(LBC)) return cudaErrorInvalidValue;
-    const size_t smem = fused_smem_bytes<T>(S, L.nfb);
+    const size_t smem = fused_smem_bytes<T>(S, lbc_nfb(LBC, P, S, NACC));
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
@@ -44,7 +44,7 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     p.btab = PolyTab<T>{static_cast<const T*>(L.btab), L.btab_first, L.btab_cells};
     p.Ftab = PolyTab<T>{static_cast<const T*>(L.Ftab), L.Ftab_first, L.Ftab_cells};
     for (int t = 0; t < NACC * S; ++t) p.W[t] = (T)L.W[t];
-    p.theta = L.theta; p.B = L.B; p.nxp = L.nxp; p.nfb = L.nfb;
+    p.theta = L.theta; p.B = L.B; p.nxp = L.nxp;
     p.maps = static_cast<T*>(L.maps); p.data = L.data; p.C0 = L.C0; p.logL = L.logL;
     kern<<<ctas, L.threads, smem, L.stream>>>(p);
     return cudaGetLastError();
@@ -57,10 +57,8 @@ cudaError_t launch_lbc(const FusedLaunch& L, FusedInfo* info, bool query_only) {
 }
 template <typename T, int S, int NACC, int P>
 cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
-    if constexpr (sizeof(T) == 4) {
-        if (L.threads <= 128) return launch_lbc<T, S, NACC, P, 0>(L, info, query_only);
-        if (L.threads <= 256) return launch_lbc<T, S, NACC, P, 1>(L, info, query_only);
-    }
+    if (L.threads <= 128) return launch_lbc<T, S, NACC, P, 0>(L, info, query_only);
+    if (L.threads <= 256) return launch_lbc<T, S, NACC, P, 1>(L, info, query_only);
     return launch_lbc<T, S, NACC, P, 2>(L, info, query_only);
 }
 

@@ -14,7 +14,7 @@ struct FusedLaunch {
     const void* Ftab; int Ftab_first, Ftab_cells;
     const double* W; int nacc;   // composite taps, nacc * s of them
     const double* theta; int B;
-    int P, nxp, nfb, mode;
+    int P, nxp, mode;
     void* maps;
     const double2* data;
     double C0;

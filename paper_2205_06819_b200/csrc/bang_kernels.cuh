@@ -390,11 +390,11 @@ BANG_D void eval_rows_any(const unsigned comps, const CellK<T>& k, const PolyTab
 // a2 + a3 for one super-row of the fused kernel (S fine rows jy0 .. jy0+S-1 = one data row): thread `vt` takes the fine
 // columns x = vt, vt + NT, ... and evaluates the S cells of each column in one iteration, so that the index arithmetic,
 // the rotation and the store address are shared by S cells and S independent dependency chains are in flight.
-// dst[(row * 4 + observable) * nfb + x].  GUARD: some of the S rows lie past the grid (zero-weight tap padding): they are
+// dst[(row * 4 + observable) * NFB + x] (NFB, the plane pitch, is a compile-time constant: immediate store offsets).  GUARD: some of the S rows lie past the grid (zero-weight tap padding): they are
 // written as zeros.
-template <typename T, int S, bool BULGE, int SHIFT, bool GUARD>
+template <typename T, int S, int NFB, bool BULGE, int SHIFT, bool GUARD>
 BANG_D void eval_superrow(const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab, T* __restrict__ dst,
-                          const int nfb, const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
+                          const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
     const T* __restrict__ bcoef = btab.coef;
     const int bfirst = btab.first, blast = btab.n_cells - 1;
     const T b0 = (T)(jy0 - k.jcy);
@@ -412,19 +412,19 @@ BANG_D void eval_superrow(const CellK<T>& k, const PolyTab<T>& btab, const T* __
                 const T xp = j == 0 ? px : fma((T)j, k.hs, px), yp = j == 0 ? py : fma((T)j, k.hc, py);
                 eval_cell<T, BULGE, SHIFT>(k, bcoef, bfirst, blast, vtab, xp, yp, vB, vV, vS, vL);
             }
-            d[(j * 4 + 0) * nfb] = vB; d[(j * 4 + 1) * nfb] = vV; d[(j * 4 + 2) * nfb] = vS; d[(j * 4 + 3) * nfb] = vL;
+            d[(j * 4 + 0) * NFB] = vB; d[(j * 4 + 1) * NFB] = vV; d[(j * 4 + 2) * NFB] = vS; d[(j * 4 + 3) * NFB] = vL;
         }
     }
 }
-template <typename T, int S, bool GUARD>
+template <typename T, int S, int NFB, bool GUARD>
 BANG_D void eval_superrow_any(const unsigned comps, const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab,
-                              T* __restrict__ dst, const int nfb, const int nfx, const int nfy, const int jy0,
+                              T* __restrict__ dst, const int nfx, const int nfy, const int jy0,
                               const int vt, const int NT) {
-    if (comps & C_BULGE) eval_superrow<T, S, true, 0, GUARD>(k, btab, vtab, dst, nfb, nfx, nfy, jy0, vt, NT);
+    if (comps & C_BULGE) eval_superrow<T, S, NFB, true, 0, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_superrow<T, S, false, 3, GUARD>(k, btab, vtab, dst, nfb, nfx, nfy, jy0, vt, NT);
-    else if (comps & C_DISC1) eval_superrow<T, S, false, 1, GUARD>(k, btab, vtab, dst, nfb, nfx, nfy, jy0, vt, NT);
-    else eval_superrow<T, S, false, 2, GUARD>(k, btab, vtab, dst, nfb, nfx, nfy, jy0, vt, NT);
+        eval_superrow<T, S, NFB, false, 3, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else if (comps & C_DISC1) eval_superrow<T, S, NFB, false, 1, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else eval_superrow<T, S, NFB, false, 2, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
 }
 
 // ---- the fused kernel ---------------------------------------------------------------------------------------------
@@ -437,7 +437,6 @@ struct FusedParams {
     const double* theta;         // [B][17]
     int B;
     int nxp;                     // data columns padded to a multiple of P
-    int nfb;                     // row-buffer width in cells (>= (nxp-1+NACC) S, multiple of 4, plus over-read slack)
     T* maps;                     // [B][4][ny][nx]
     const double2* data;         // [ny][4][P][nxp/P] {d, 1/e} of pixel group P + i (1/e = 0 where masked or padded)
     double C0;                   // sum over used pixels of -1/2 ln(2 pi e^2)
@@ -491,14 +490,21 @@ BANG_D double inv_ml(double x) { return 1.0 / x; }
 // MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike)
 // LBC: launch-bound class = the CTA-size bracket the kernel is compiled for, which fixes its register budget:
 //   0: <= 128 threads, 7 (P = 2) or 5 (P = 4) CTAs per SM;  1: <= 256 threads, 3 or 2 CTAs per SM;  2: <= 512 threads.
-// fp64 mode is compiled for class 2 only.
+// The class also fixes the row-buffer pitch (lbc_nfb), hence the shared memory per CTA.
 #ifndef BANG_B1P4
 #define BANG_B1P4 2
 #endif
 constexpr int lbc_threads(int lbc) { return lbc == 0 ? 128 : (lbc == 1 ? 256 : 512); }
-constexpr int lbc_blocks(int lbc, int P) { return lbc == 0 ? (P == 2 ? 7 : 5) : (lbc == 1 ? (P == 2 ? 3 : BANG_B1P4) : 1); }
+// Row-buffer plane pitch in cells, a compile-time constant of the instantiation (so that the 4 S planes sit at immediate
+// offsets): the widest row the class can hold -- nxp <= threads P / 4 data columns -- i.e. (nxp - 1 + NACC) S cells,
+// rounded up to a multiple of 4, plus 4 cells of over-read slack for the vector loads.
+constexpr int lbc_nfb(int lbc, int P, int S, int NACC) { return ((lbc_threads(lbc) * P / 4 - 1 + NACC) * S + 3) / 4 * 4 + 4; }
+constexpr int lbc_blocks(int lbc, int P, bool f64) {
+    return f64 ? (lbc == 0 ? 4 : (lbc == 1 ? 2 : 1))          // fp64 mode: 128 registers in every class
+               : (lbc == 0 ? (P == 2 ? 7 : 5) : (lbc == 1 ? (P == 2 ? 3 : BANG_B1P4) : 1));
+}
 template <typename T, int S, int NACC, int P, int MODE, int LBC>
-__global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P)) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
+__global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T) == 8)) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     constexpr int RUN = (P - 1 + NACC) * S;          // fine cells one thread reads per row for its P data pixels
     constexpr int RUN_BYTES = P * S * (int)sizeof(T);   // byte stride between the runs of neighbouring threads
@@ -508,7 +514,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P)) k_fused(
     constexpr size_t off_tab = (sizeof(ThetaC<T>) + 15) / 16 * 16;
     T* vtab = reinterpret_cast<T*>(smem_raw + off_tab);
     T* rowbuf = vtab + (size_t)kMaxOct * (1 << TabCfg<T>::M) * NC;
-    const int nfb = p.nfb;
+    constexpr int nfb = lbc_nfb(LBC, P, S, NACC);
     double* red = reinterpret_cast<double*>(rowbuf + (size_t)S * 4 * nfb);
 
     const GridC& g = p.g;
@@ -551,8 +557,8 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P)) k_fused(
             // the per-theta constants are re-read from shared memory for every super-row (a handful of broadcast loads)
             // so that they do not occupy registers during the PSF phase
             const CellK<T> k = load_cellk<T>(c);
-            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, false>(g.comps, k, p.btab, vtab, rowbuf, nfb, g.nfx, g.nfy, sr * S, vt, NT);
-            else eval_superrow_any<T, S, true>(g.comps, k, p.btab, vtab, rowbuf, nfb, g.nfx, g.nfy, sr * S, vt, NT);
+            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, false>(g.comps, k, p.btab, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            else eval_superrow_any<T, S, nfb, true>(g.comps, k, p.btab, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
             vt = vt + 32 < NT ? vt + 32 : vt + 32 - NT;      // rotate the column ownership by one warp: the ragged last
                                                              // pass then falls on a different warp (scheduler) each time
             __syncthreads();
