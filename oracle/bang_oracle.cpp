@@ -133,6 +133,66 @@ double rho_vr2(double r, double Mb, double Rb) {
     return kG * Mb * Mb / (2 * kPi * Rb * Rb * Rb * Rb) * T5(Rb / (r + Rb));
 }
 
+// ---- Appendix B: Jaffe bulge (reading J) -----------------------------
+// eq. B1: rho_b = M_b R_b / (4 pi r^2 (r + R_b)^2);  M(<r) = M_b r/(r + R_b);  eq. B2: v_c^2 = G M_b/(r + R_b).
+double vc2_jaffe(double r, double M, double a) { return kG * M / (r + a); }
+
+// eq. B4: Sigma_b(R) = M_b/R_b^2 * SigmaTildeJ(s),
+// SigmaTildeJ(s) = 1/(4 s) + [1 - (2 - s^2) X(s)] / (2 pi (1 - s^2)),  X(s) of eq. 5.
+template <typename T> T jaffe_sigma_tilde_T(T s) {
+    const T one = 1, pi = T(4) * (sizeof(T) == 8 ? T(std::atan(1.0)) : T(atanq((__float128)1)));
+    return one / (T(4) * s) + (one - (T(2) - s * s) * hernquist_X<T>(s)) / (T(2) * pi * (one - s * s));
+}
+// Removable singularity at s = 1 (value 1/4 - 2/(3 pi)): Taylor series for |s-1| < 1e-7.  For s >> 1 the two terms
+// cancel to Sigma ~ 1/(8 s^3) (relative loss ~ eps s^2), so binary128 is used for every s > 0.5.
+double jaffe_sigma_tilde(double s) {
+    double e = s - 1.0;
+    if (std::fabs(e) < 1e-7) return (0.25 - 2.0 / (3.0 * kPi)) - 0.0802347273686449752 * e + 0.116613000075362963 * e * e;
+    if (s > 0.5) return (double)jaffe_sigma_tilde_T<__float128>((__float128)s);
+    return jaffe_sigma_tilde_T<double>(s);
+}
+
+// Isotropic Jeans integral of eqs. B1-B2: rho_b v_r^2 = int_r^inf rho_b G M(<x)/x^2 dx
+//   = G M_b^2/(4 pi R_b^4) * J3(u),  u = R_b/(r + R_b),
+//   J3 = int_t^inf dt'/(t'^3 (1+t')^3) = 1/(2t^2) - 3/t - 3/(1+t) - 1/(2(1+t)^2) + 6 ln(1 + 1/t),  t = r/R_b
+//      = int_0^u u'^4/(1-u')^3 du' = sum_{n>=5} (n-3)(n-4)/2 u^n/n      (the closed form cancels like t^-5 for t >> 1).
+// Equals rho_b x eq. B3 with the sign of B3's braces reversed and a = R_b (reading J; pinned in tests).
+double J3(double u) {
+    if (u <= 0.0) return 0.0;
+    if (u < 0.5) {
+        double un = u * u * u * u * u, sum = 0.0;
+        for (int n = 5; n < 400; ++n) {
+            double term = 0.5 * (n - 3) * (n - 4) * un / n;
+            sum += term;
+            if (term < 1e-18 * sum) break;
+            un *= u;
+        }
+        return sum;
+    }
+    double t = (1.0 - u) / u;
+    return 1.0 / (2 * t * t) - 3.0 / t - 3.0 / (1 + t) - 1.0 / (2 * (1 + t) * (1 + t)) + 6.0 * std::log1p(1.0 / t);
+}
+double rho_vr2_jaffe(double r, double Mb, double Rb) {
+    return kG * Mb * Mb / (4 * kPi * Rb * Rb * Rb * Rb) * J3(Rb / (r + Rb));
+}
+// eq. B3 with reading J's corrections (a = R_b, sign), in binary128: pin only.
+double vr2_jaffe_corrected(double r, double Mb, double Rb) {
+    __float128 x = (__float128)r / Rb;
+    __float128 br = 6 * logq(1 + 1 / x) - 3 / x - (6 * x + 7) / (2 * (x + 1) * (x + 1)) + 1 / (2 * x * x);
+    return (double)((__float128)(kG * Mb / Rb) * x * x * (1 + x) * (1 + x) * br);
+}
+// eq. B5 times Sigma_b: Sigma_b sigma_b^2 = G M_b^2/(4 pi R_b^3) * ITildeJ(s),
+// ITildeJ = [pi/(2s) + 11 - (13/2) pi s - 12 s^2 + 6 pi s^3 - X(s)(6 - 19 s^2 + 12 s^4)] / (1 - s^2); binary128.
+// NOT on the model path: the pin for the N_J-node quadrature below.
+double jaffe_I_tilde_closed(double sd) {
+    double e = sd - 1.0;
+    if (std::fabs(e) < 1e-5) return 0.0545737385894705218 - 0.153685581666989383 * e + 0.2755582315567978 * e * e;
+    __float128 s = sd, s2 = s * s, pi = 4 * atanq((__float128)1);
+    __float128 X = hernquist_X<__float128>(s);
+    __float128 num = pi / (2 * s) + 11 - (__float128)13 / 2 * pi * s - 12 * s2 + 6 * pi * s2 * s - X * (6 - 19 * s2 + 12 * s2 * s2);
+    return (double)(num / (1 - s2));
+}
+
 // ---- Gauss-Legendre nodes on (-1,1) ----------------------------------------------------------
 void gauss_legendre(int n, double *x, double *w) {
     for (int i = 0; i < (n + 1) / 2; ++i) {
@@ -168,6 +228,19 @@ double Ib_quadrature(double R, double Mb, double Rb, int NJ, const double *glx, 
         sum += wt * dzdt * T5(Rb / (Rb + r));
     }
     return kG * Mb * Mb / (2 * kPi * Rb * Rb * Rb * Rb) * 2.0 * sum;
+}
+
+// The same N_J-node rule for the Jaffe bulge: I_b(R) = 2 int_0^inf rho_b v_r^2 dz with rho_b v_r^2 of rho_vr2_jaffe.
+double Ib_quadrature_jaffe(double R, double Mb, double Rb, int NJ, const double *glx, const double *glw) {
+    double L = std::sqrt(R * R + Rb * Rb), sum = 0.0;
+    for (int k = 0; k < NJ; ++k) {
+        double t = 0.5 * (glx[k] + 1.0), wt = 0.5 * glw[k];
+        double z = L * t * t / (1.0 - t);
+        double dzdt = L * t * (2.0 - t) / ((1.0 - t) * (1.0 - t));
+        double r = std::sqrt(R * R + z * z);
+        sum += wt * dzdt * J3(Rb / (Rb + r));
+    }
+    return kG * Mb * Mb / (4 * kPi * Rb * Rb * Rb * Rb) * 2.0 * sum;
 }
 
 // ---- eq. 9 (reading D): v_c^2 = (2 G M_d / R_d) F(r / 2R_d), F(y) = y^2 [I0 K0 - I1 K1](y) ------
@@ -256,7 +329,8 @@ struct Setup {
     int nx, ny, s, rk, nfx, nfy, NJ;
     double pix, kappa;
     unsigned comps;
-    int halo_profile;
+    int halo_profile;                  // 0 Hernquist (paper), 1 NFW (reading H)
+    int bulge_profile;                 // 0 Hernquist (paper default), 1 Jaffe (App. B)
     std::vector<double> taps, glx, glw;
 };
 
@@ -277,12 +351,15 @@ void psf_taps(double sigma_pix, int s, double trunc, std::vector<double> &g) {
     for (double &v : g) v /= sum;
 }
 
+// profiles: bits 0-7 halo profile, bits 8-15 bulge profile
 bool make_setup(Setup &S, int nx, int ny, double pix, int s, double dist_mpc, double sigma_pix,
-                double trunc, unsigned comps, int halo_profile, int NJ) {
+                double trunc, unsigned comps, int profiles, int NJ) {
+    const int halo_profile = profiles & 0xff, bulge_profile = (profiles >> 8) & 0xff;
+    if (halo_profile > 1 || bulge_profile > 1) return false;
     if (nx < 1 || ny < 1 || s < 1 || !(pix > 0) || !(dist_mpc > 0) || sigma_pix < 0 || NJ < 1) return false;
     if (!(comps & (C_BULGE | C_DISC1 | C_DISC2))) return false;
     S.nx = nx; S.ny = ny; S.s = s; S.pix = pix; S.kappa = dist_mpc * kArcsecKpcPerMpc;
-    S.comps = comps; S.halo_profile = halo_profile; S.NJ = NJ;
+    S.comps = comps; S.halo_profile = halo_profile; S.bulge_profile = bulge_profile; S.NJ = NJ;
     psf_taps(sigma_pix, s, trunc, S.taps);
     S.rk = (int(S.taps.size()) - 1) / 2;
     S.nfx = nx * s + 2 * S.rk; S.nfy = ny * s + 2 * S.rk;
@@ -308,10 +385,14 @@ void fine_cell(const Setup &S, const Theta &t, int Jx, int Jy, double out[4]) {
     double cosphi = xp / r;
     // 4. bulge: eq. 4 and eq. 6 (first form, N_J nodes)
     double Sb = 0.0, Ib = 0.0, vc2 = 0.0;
-    if (S.comps & C_BULGE) {
+    if ((S.comps & C_BULGE) && S.bulge_profile == 0) {
         Sb = t.Mb / (2 * kPi * t.Rb * t.Rb) * sigma_tilde(R / t.Rb);
         Ib = Ib_quadrature(R, t.Mb, t.Rb, S.NJ, S.glx.data(), S.glw.data());
         vc2 += vc2_hernquist(r, t.Mb, t.Rb);
+    } else if (S.comps & C_BULGE) {            // Jaffe: eq. B4, B2 and the l.o.s. integral of rho_b v_r^2 (B1, B3)
+        Sb = t.Mb / (t.Rb * t.Rb) * jaffe_sigma_tilde(R / t.Rb);
+        Ib = Ib_quadrature_jaffe(R, t.Mb, t.Rb, S.NJ, S.glx.data(), S.glw.data());
+        vc2 += vc2_jaffe(r, t.Mb, t.Rb);
     }
     // 5. discs: eq. 7-8;  6. circular speed: eq. 2, 9, 10
     double Sd[2] = {0.0, 0.0};
@@ -428,6 +509,17 @@ double bo_nfw_mu(double x) { return nfw_mu(x); }
 double bo_nfw_r200(double M200) { return nfw_r200(M200); }
 double bo_vc2_nfw(double r, double M200, double c) { return vc2_nfw(r, M200, c); }
 double bo_hernquist_Sigma(double R, double Mb, double Rb) { return Mb / (2 * kPi * Rb * Rb) * sigma_tilde(R / Rb); }
+double bo_jaffe_sigma_tilde(double s) { return jaffe_sigma_tilde(s); }
+double bo_jaffe_I_tilde_closed(double s) { return jaffe_I_tilde_closed(s); }
+double bo_J3(double u) { return J3(u); }
+double bo_rho_vr2_jaffe(double r, double Mb, double Rb) { return rho_vr2_jaffe(r, Mb, Rb); }
+double bo_vr2_jaffe_corrected(double r, double Mb, double Rb) { return vr2_jaffe_corrected(r, Mb, Rb); }
+double bo_vc2_jaffe(double r, double M, double a) { return vc2_jaffe(r, M, a); }
+double bo_Ib_quadrature_jaffe(double R, double Mb, double Rb, int NJ) {
+    std::vector<double> x(NJ), w(NJ);
+    gauss_legendre(NJ, x.data(), w.data());
+    return Ib_quadrature_jaffe(R, Mb, Rb, NJ, x.data(), w.data());
+}
 double bo_G() { return kG; }
 double bo_kappa(double dist_mpc) { return dist_mpc * kArcsecKpcPerMpc; }
 
@@ -442,9 +534,9 @@ int bo_psf_taps(double sigma_pix, int s, double trunc, double *g /*[2 r_k + 1]*/
 // ---- maps ----
 // fine: [4][N_y s + 2 r_k][N_x s + 2 r_k], un-convolved B_tot, v_los, sigma_los, <L/M>. Returns 0, or -1 (bad setup), -2 (theta out of domain).
 int bo_model_fine(const double *theta, int nx, int ny, double pix, int s, double dist_mpc, double sigma_pix,
-                  double trunc, unsigned comps, int halo_profile, int NJ, double *fine) {
+                  double trunc, unsigned comps, int profiles, int NJ, double *fine) {
     Setup S;
-    if (!make_setup(S, nx, ny, pix, s, dist_mpc, sigma_pix, trunc, comps, halo_profile, NJ)) return -1;
+    if (!make_setup(S, nx, ny, pix, s, dist_mpc, sigma_pix, trunc, comps, profiles, NJ)) return -1;
     Theta t = decode(theta, comps);
     if (!t.valid) return -2;
     fine_maps(S, t, fine);
@@ -461,9 +553,9 @@ int bo_convolve_rebin(const double *fine, int nx, int ny, int s, double sigma_pi
 
 // maps: [B][4][ny][nx] = B [Lsun/pc^2], v_los [km/s], sigma_los [km/s], M/L.  Out-of-domain theta -> NaN.
 int bo_model_maps(const double *theta, int B, int nx, int ny, double pix, int s, double dist_mpc,
-                  double sigma_pix, double trunc, unsigned comps, int halo_profile, int NJ, double *maps) {
+                  double sigma_pix, double trunc, unsigned comps, int profiles, int NJ, double *maps) {
     Setup S;
-    if (!make_setup(S, nx, ny, pix, s, dist_mpc, sigma_pix, trunc, comps, halo_profile, NJ)) return -1;
+    if (!make_setup(S, nx, ny, pix, s, dist_mpc, sigma_pix, trunc, comps, profiles, NJ)) return -1;
     std::vector<double> fine;
     for (int b = 0; b < B; ++b) model_one(S, theta + 17 * (size_t)b, maps + (size_t)b * 4 * nx * ny, fine);
     return 0;
@@ -483,10 +575,10 @@ double bo_loglike_of_maps(const double *maps, const double *data, const double *
 
 // logL[B]; out-of-domain theta -> -inf.  maps_out may be NULL, else receives [B][4][ny][nx].
 int bo_loglike(const double *theta, int B, int nx, int ny, double pix, int s, double dist_mpc, double sigma_pix,
-               double trunc, unsigned comps, int halo_profile, int NJ, const double *data, const double *err,
+               double trunc, unsigned comps, int profiles, int NJ, const double *data, const double *err,
                const unsigned char *mask, double *logL, double *maps_out) {
     Setup S;
-    if (!make_setup(S, nx, ny, pix, s, dist_mpc, sigma_pix, trunc, comps, halo_profile, NJ)) return -1;
+    if (!make_setup(S, nx, ny, pix, s, dist_mpc, sigma_pix, trunc, comps, profiles, NJ)) return -1;
     std::vector<double> fine, maps((size_t)4 * nx * ny);
     for (int b = 0; b < B; ++b) {
         Theta t = decode(theta + 17 * (size_t)b, comps);

@@ -18,6 +18,7 @@ _SO = os.path.join(_HERE, "libbang_oracle.so")
 
 BULGE, DISC1, DISC2, HALO = 1, 2, 4, 8
 HALO_HERNQUIST, HALO_NFW = 0, 1
+BULGE_HERNQUIST, BULGE_JAFFE = 0, 1
 
 
 def build(force: bool = False) -> str:
@@ -45,6 +46,9 @@ def lib():
             "bo_vc2_hernquist": [_d, _d, _d], "bo_vc2_expdisc": [_d, _d, _d], "bo_nfw_mu": [_d],
             "bo_nfw_r200": [_d], "bo_vc2_nfw": [_d, _d, _d], "bo_hernquist_Sigma": [_d, _d, _d],
             "bo_G": [], "bo_kappa": [_d],
+            "bo_jaffe_sigma_tilde": [_d], "bo_jaffe_I_tilde_closed": [_d], "bo_J3": [_d],
+            "bo_rho_vr2_jaffe": [_d, _d, _d], "bo_vr2_jaffe_corrected": [_d, _d, _d], "bo_vc2_jaffe": [_d, _d, _d],
+            "bo_Ib_quadrature_jaffe": [_d, _d, _d, _i],
         }.items():
             f = getattr(L, name)
             f.argtypes, f.restype = args, _d
@@ -53,7 +57,7 @@ def lib():
         L.bo_gauss_legendre.argtypes, L.bo_gauss_legendre.restype = [_i, _dp, _dp], None
         L.bo_psf_halfwidth.argtypes, L.bo_psf_halfwidth.restype = [_d, _i, _d], _i
         L.bo_psf_taps.argtypes, L.bo_psf_taps.restype = [_d, _i, _d, _dp], _i
-        cfg = [_i, _i, _d, _i, _d, _d, _d, _u, _i, _i]   # nx ny pix s dist sigma trunc comps halo NJ
+        cfg = [_i, _i, _d, _i, _d, _d, _d, _u, _i, _i]   # nx ny pix s dist sigma trunc comps profiles NJ
         L.bo_model_fine.argtypes, L.bo_model_fine.restype = [_dp] + cfg + [_dp], _i
         L.bo_convolve_rebin.argtypes, L.bo_convolve_rebin.restype = [_dp, _i, _i, _i, _d, _d, _dp], _i
         L.bo_model_maps.argtypes, L.bo_model_maps.restype = [_dp, _i] + cfg + [_dp], _i
@@ -73,10 +77,12 @@ def get_threads() -> int:
 
 
 def _cfg(cfg):
-    """cfg: dict with nx ny pix_arcsec supersample dist_mpc sigma_pix trunc_nsigma components halo_profile jeans_nodes."""
+    """cfg: dict with nx ny pix_arcsec supersample dist_mpc sigma_pix trunc_nsigma components halo_profile
+    [bulge_profile] jeans_nodes.  The two profile switches travel in one int: halo | bulge << 8."""
     return (int(cfg["nx"]), int(cfg["ny"]), float(cfg["pix_arcsec"]), int(cfg["supersample"]),
             float(cfg["dist_mpc"]), float(cfg["sigma_pix"]), float(cfg.get("trunc_nsigma", 3.0)),
-            int(cfg["components"]), int(cfg.get("halo_profile", 0)), int(cfg["jeans_nodes"]))
+            int(cfg["components"]), int(cfg.get("halo_profile", 0)) | (int(cfg.get("bulge_profile", 0)) << 8),
+            int(cfg["jeans_nodes"]))
 
 
 def psf_halfwidth(cfg) -> int:
