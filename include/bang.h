@@ -55,7 +55,9 @@ extern "C" {
 #define BANG_DISC2 4u
 #define BANG_HALO  8u
 
-#define BANG_BULGE_HERNQUIST 0   /* the paper's default, eq. 1-6 */
+#define BANG_BULGE_HERNQUIST 0   /* the paper's default, eq. 1-6 (PAPER.md:78-105) */
+#define BANG_BULGE_JAFFE     1   /* Appendix B: eq. B1, B2, B4; Sigma_b sigma_b^2 = the N_J-node l.o.s.
+                                    integral of eq. B1 x B3 (B3 as corrected by reading J), which eq. B5 pins */
 #define BANG_HALO_HERNQUIST  0   /* the paper's halo: eq. 2 with (M_h, R_h) */
 #define BANG_HALO_NFW        1   /* BASELINE.json configs 2-5: (log10 M200, c), H0 = 70 km/s/Mpc (reading H) */
 #define BANG_FP32 0              /* fp32 model arithmetic; residuals and logL accumulation in fp64 */
@@ -77,7 +79,7 @@ typedef struct {
 
 typedef struct {
     unsigned components;   /* BANG_BULGE | BANG_DISC1 | BANG_DISC2 | BANG_HALO; at least one luminous component */
-    int bulge_profile;     /* BANG_BULGE_HERNQUIST */
+    int bulge_profile;     /* BANG_BULGE_HERNQUIST or BANG_BULGE_JAFFE */
     int halo_profile;      /* BANG_HALO_HERNQUIST or BANG_HALO_NFW */
     int jeans_nodes;       /* N_J >= 1: nodes of the Gauss-Legendre rule for the bulge Jeans l.o.s. integral (reading B) */
     int precision;         /* BANG_FP32 or BANG_FP64 */

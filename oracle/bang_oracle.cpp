@@ -153,13 +153,14 @@ double jaffe_sigma_tilde(double s) {
 }
 
 // Isotropic Jeans integral of eqs. B1-B2: rho_b v_r^2 = int_r^inf rho_b G M(<x)/x^2 dx
-//   = G M_b^2/(4 pi R_b^4) * J3(u),  u = R_b/(r + R_b),
+//   = G M_b^2/(4 pi R_b^4) * J3(t),  t = r/R_b,  u = R_b/(r + R_b) = 1/(1+t),
 //   J3 = int_t^inf dt'/(t'^3 (1+t')^3) = 1/(2t^2) - 3/t - 3/(1+t) - 1/(2(1+t)^2) + 6 ln(1 + 1/t),  t = r/R_b
 //      = int_0^u u'^4/(1-u')^3 du' = sum_{n>=5} (n-3)(n-4)/2 u^n/n      (the closed form cancels like t^-5 for t >> 1).
 // Equals rho_b x eq. B3 with the sign of B3's braces reversed and a = R_b (reading J; pinned in tests).
-double J3(double u) {
-    if (u <= 0.0) return 0.0;
-    if (u < 0.5) {
+double J3(double t) {                          // argument: t = r/R_b (not u, which loses t for t << 1)
+    if (!(t < INFINITY)) return 0.0;
+    if (t > 1.0) {
+        double u = 1.0 / (1.0 + t);
         double un = u * u * u * u * u, sum = 0.0;
         for (int n = 5; n < 400; ++n) {
             double term = 0.5 * (n - 3) * (n - 4) * un / n;
@@ -169,11 +170,10 @@ double J3(double u) {
         }
         return sum;
     }
-    double t = (1.0 - u) / u;
     return 1.0 / (2 * t * t) - 3.0 / t - 3.0 / (1 + t) - 1.0 / (2 * (1 + t) * (1 + t)) + 6.0 * std::log1p(1.0 / t);
 }
 double rho_vr2_jaffe(double r, double Mb, double Rb) {
-    return kG * Mb * Mb / (4 * kPi * Rb * Rb * Rb * Rb) * J3(Rb / (r + Rb));
+    return kG * Mb * Mb / (4 * kPi * Rb * Rb * Rb * Rb) * J3(r / Rb);
 }
 // eq. B3 with reading J's corrections (a = R_b, sign), in binary128: pin only.
 double vr2_jaffe_corrected(double r, double Mb, double Rb) {
@@ -238,7 +238,7 @@ double Ib_quadrature_jaffe(double R, double Mb, double Rb, int NJ, const double 
         double z = L * t * t / (1.0 - t);
         double dzdt = L * t * (2.0 - t) / ((1.0 - t) * (1.0 - t));
         double r = std::sqrt(R * R + z * z);
-        sum += wt * dzdt * J3(Rb / (Rb + r));
+        sum += wt * dzdt * J3(r / Rb);
     }
     return kG * Mb * Mb / (4 * kPi * Rb * Rb * Rb * Rb) * 2.0 * sum;
 }
@@ -511,7 +511,7 @@ double bo_vc2_nfw(double r, double M200, double c) { return vc2_nfw(r, M200, c);
 double bo_hernquist_Sigma(double R, double Mb, double Rb) { return Mb / (2 * kPi * Rb * Rb) * sigma_tilde(R / Rb); }
 double bo_jaffe_sigma_tilde(double s) { return jaffe_sigma_tilde(s); }
 double bo_jaffe_I_tilde_closed(double s) { return jaffe_I_tilde_closed(s); }
-double bo_J3(double u) { return J3(u); }
+double bo_J3(double t) { return J3(t); }
 double bo_rho_vr2_jaffe(double r, double Mb, double Rb) { return rho_vr2_jaffe(r, Mb, Rb); }
 double bo_vr2_jaffe_corrected(double r, double Mb, double Rb) { return vr2_jaffe_corrected(r, Mb, Rb); }
 double bo_vc2_jaffe(double r, double M, double a) { return vc2_jaffe(r, M, a); }

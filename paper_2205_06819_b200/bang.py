@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libbang.so")
 
 BULGE, DISC1, DISC2, HALO = 1, 2, 4, 8
 HALO_HERNQUIST, HALO_NFW = 0, 1
+BULGE_HERNQUIST, BULGE_JAFFE = 0, 1
 FP32, FP64 = 0, 1
 NTHETA = 17
 OK, EINVAL, ENOMEM, ECUDA, ENODATA = 0, -1, -2, -3, -4
@@ -91,7 +92,7 @@ class Context:
         self.nx, self.ny, self.s = int(cfg["nx"]), int(cfg["ny"]), int(cfg["supersample"])
         g = Grid(self.nx, self.ny, float(cfg["pix_arcsec"]), self.s, float(cfg["dist_mpc"]))
         p = Psf(float(cfg["sigma_pix"]), float(cfg.get("trunc_nsigma", 3.0)))
-        m = Model(int(cfg["components"]), 0, int(cfg.get("halo_profile", 0)), int(cfg["jeans_nodes"]),
+        m = Model(int(cfg["components"]), int(cfg.get("bulge_profile", 0)), int(cfg.get("halo_profile", 0)), int(cfg["jeans_nodes"]),
                   FP64 if prec == "fp64" else FP32)
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         h = C.c_void_p()

@@ -109,10 +109,11 @@ void make_fit(int D, FitC& fit) {
 }
 
 // ---- one-off kernels: the scale-free tables (K0) ---------------------------------------------
-// which = 0: Hernquist SigmaTilde(s) and the N_J-node Jeans integral J(s), at u = s^2;  which = 1: Freeman F(y), u = y^2
+// which = 0: the bulge's SigmaTilde(s) and N_J-node Jeans integral J(s) (Hernquist or Jaffe), at u = s^2;
+// which = 1: Freeman F(y), u = y^2
 template <typename T>
-__global__ void k_univ_nodes(int which, int first, int n_cells, FitC fit, int NJ, const double* __restrict__ glx,
-                             const double* __restrict__ glw, double* __restrict__ vals) {
+__global__ void k_univ_nodes(int which, int bulge_profile, int first, int n_cells, FitC fit, int NJ,
+                             const double* __restrict__ glx, const double* __restrict__ glw, double* __restrict__ vals) {
     constexpr int NC = TabCfg<T>::D + 1;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_cells * NC) return;
@@ -121,8 +122,8 @@ __global__ void k_univ_nodes(int which, int first, int n_cells, FitC fit, int NJ
     tab_interval<T>(first + cell, lo, width);
     const double x = sqrt(lo + 0.5 * width * (fit.tnode[k] + 1.0));
     if (which == 0) {
-        vals[(cell * 2 + 0) * NC + k] = sigma_tilde(x);
-        vals[(cell * 2 + 1) * NC + k] = jeans_J(x, NJ, glx, glw);
+        vals[(cell * 2 + 0) * NC + k] = bulge_profile == 1 ? jaffe_sigma_tilde(x) : sigma_tilde(x);
+        vals[(cell * 2 + 1) * NC + k] = bulge_profile == 1 ? jaffe_jeans_J(x, NJ, glx, glw) : jeans_J(x, NJ, glx, glw);
     } else {
         vals[cell * NC + k] = freeman_F(x);
     }
@@ -189,9 +190,9 @@ int build_universal(bang_ctx* ctx, const double* glx_dev, const double* glw_dev)
     CU(cudaMalloc(&ctx->btab, nb * sizeof(T)));
     CU(cudaMalloc(&ctx->Ftab, nf * sizeof(T)));
     const int th = 128;
-    k_univ_nodes<T><<<(ctx->btab_cells * NC + th - 1) / th, th, 0, ctx->stream>>>(0, ctx->btab_first, ctx->btab_cells, ctx->fit,
+    k_univ_nodes<T><<<(ctx->btab_cells * NC + th - 1) / th, th, 0, ctx->stream>>>(0, ctx->model.bulge_profile, ctx->btab_first, ctx->btab_cells, ctx->fit,
                                                                                 ctx->model.jeans_nodes, glx_dev, glw_dev, vals);
-    k_univ_nodes<T><<<(ctx->Ftab_cells * NC + th - 1) / th, th, 0, ctx->stream>>>(1, ctx->Ftab_first, ctx->Ftab_cells, ctx->fit, 0,
+    k_univ_nodes<T><<<(ctx->Ftab_cells * NC + th - 1) / th, th, 0, ctx->stream>>>(1, 0, ctx->Ftab_first, ctx->Ftab_cells, ctx->fit, 0,
                                                                                 nullptr, nullptr, vals + nb);
     k_univ_fit<T><<<(ctx->btab_cells * 2 + th - 1) / th, th, 0, ctx->stream>>>(ctx->btab_cells * 2, ctx->fit, vals,
                                                                              static_cast<T*>(ctx->btab));
@@ -297,7 +298,7 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     if (!(psf->sigma_pix >= 0) || !(psf->trunc_nsigma >= 0) || !std::isfinite(psf->sigma_pix) || !std::isfinite(psf->trunc_nsigma))
         return BANG_EINVAL;
     if (!(model->components & (BANG_BULGE | BANG_DISC1 | BANG_DISC2)) || (model->components & ~15u)) return BANG_EINVAL;
-    if (model->bulge_profile != BANG_BULGE_HERNQUIST) return BANG_EINVAL;
+    if (model->bulge_profile != BANG_BULGE_HERNQUIST && model->bulge_profile != BANG_BULGE_JAFFE) return BANG_EINVAL;
     if (model->halo_profile != BANG_HALO_HERNQUIST && model->halo_profile != BANG_HALO_NFW) return BANG_EINVAL;
     if (model->jeans_nodes < 1 || model->jeans_nodes > 4096) return BANG_EINVAL;
     if (model->precision != BANG_FP32 && model->precision != BANG_FP64) return BANG_EINVAL;
@@ -327,7 +328,7 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     g.jsx = rk - 0.5 + 0.5 * grid->nx * s; g.jsy = rk - 0.5 + 0.5 * grid->ny * s;
     g.spx = s / grid->pix_arcsec;
     g.h = grid->pix_arcsec * grid->dist_mpc * kKpcPerArcsecPerMpc / s;
-    g.comps = model->components; g.halo_profile = model->halo_profile;
+    g.comps = model->components; g.halo_profile = model->halo_profile; g.bulge_profile = model->bulge_profile;
 
     // eq. 21 on the fine grid, separable (reading F): g[m] = exp(-m^2/(2 sigma_f^2)), normalised;
     // composed with the s-cell box of the rebin: W[t] = (1/s) sum_{b<s} g[t - b], t = 0 .. 2 r_k + s - 1.

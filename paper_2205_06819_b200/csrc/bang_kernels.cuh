@@ -68,7 +68,8 @@ struct GridC {
     double spx;                  // s / pix_arcsec: fine cells per arcsec
     double h;                    // fine cell size [kpc]
     unsigned comps;
-    int halo_profile;
+    int halo_profile;            // 0 Hernquist (paper), 1 NFW (reading H)
+    int bulge_profile;           // 0 Hernquist (paper default), 1 Jaffe (App. B)
 };
 
 struct FitC {                    // Chebyshev-node fit of degree D: nodes t_k and the inverse Vandermonde matrix
@@ -104,7 +105,10 @@ BANG_D double freeman_F_tab(const PolyTab<T>& Ftab, double y2) {
 template <typename T>
 BANG_D double vc2_total(const ThetaD& d, const GridC& g, const PolyTab<T>& Ftab, double r) {
     double v2 = 0.0;
-    if (g.comps & C_BULGE) { const double a = r + d.Rb; v2 += d.GMb * r / (a * a); }
+    if (g.comps & C_BULGE) {
+        const double a = r + d.Rb;
+        v2 += g.bulge_profile == 1 ? d.GMb / a : d.GMb * r / (a * a);      // eq. B2 / eq. 2
+    }
 #pragma unroll
     for (int j = 0; j < 2; ++j)
         if (g.comps & (j ? C_DISC2 : C_DISC1)) {
@@ -170,13 +174,18 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, ThetaC<T
     // bulge: eq. 1-6
     c.invRb2 = T(1); c.ampBb = T(0); c.ampIb = T(0); c.MLb = T(1);
     d.GMb = 0.0; d.Rb = 1.0;
-    if (comps & C_BULGE) {
+    if (comps & C_BULGE) {      // eq. 1-6 (Hernquist) or App. B (Jaffe): both scale-free in s = R/R_b
         const double Mb = exp10(th[4]), Rb = th[5], MLb = th[12];
         const double inv = 1.0 / (Rb * Rb);
         if (!(R2min * inv * lo_m >= ldexp(1.0, kBulgeOctLo)) || !(R2max * inv * hi_m < ldexp(1.0, kBulgeOctHi))) return;
         c.invRb2 = (T)inv;
-        c.ampBb = (T)(Mb / (2.0 * kPi * Rb * Rb) / MLb * 1e-6);                          // eq. 4, in Lsun/pc^2
-        c.ampIb = (T)(kG * Mb * Mb / (2.0 * kPi * Rb * Rb * Rb) * 2.0 / MLb * 1e-6);     // eq. 6 first form
+        if (g.bulge_profile == 1) {
+            c.ampBb = (T)(Mb / (Rb * Rb) / MLb * 1e-6);                                  // eq. B4, in Lsun/pc^2
+            c.ampIb = (T)(kG * Mb * Mb / (4.0 * kPi * Rb * Rb * Rb) * 2.0 / MLb * 1e-6); // l.o.s. integral of B1 x B3
+        } else {
+            c.ampBb = (T)(Mb / (2.0 * kPi * Rb * Rb) / MLb * 1e-6);                      // eq. 4, in Lsun/pc^2
+            c.ampIb = (T)(kG * Mb * Mb / (2.0 * kPi * Rb * Rb * Rb) * 2.0 / MLb * 1e-6); // eq. 6 first form
+        }
         c.MLb = (T)MLb;
         d.GMb = kG * Mb; d.Rb = Rb;
     }

@@ -92,6 +92,80 @@ BANG_HD double sigma_tilde(double s) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Jaffe bulge (Appendix B; reading J).
+// eq. B4: Sigma_b = M_b/R_b^2 SigmaTildeJ(s),  SigmaTildeJ = 1/(4s) + [1 - (2 - s^2) X(s)]/(2 pi (1 - s^2)).
+//   |1 - s^2| < 1/4: with w = 1 - s^2 and X = sum_n w^n/(2n+1),  [1 - (1+w) X]/w = -sum_{n>=1} 4n/(4n^2-1) w^(n-1);
+//   s >= 8: the two terms cancel to ~1/(8 s^3); use the projection of the large-r expansion of eq. B1 term by term,
+//           rho = (1/4 pi) sum_k (-1)^k (k+1) r^-(k+4),  2 int_0^inf (s^2+z^2)^(-m/2) dz = c_m s^(1-m),
+//           c_4 = pi/2, c_5 = 4/3, c_(m+2) = c_m (m-1)/m.
+BANG_HD double jaffe_sigma_tilde(double s) {
+    const double w = 1.0 - s * s;
+    if (fabs(w) < 0.25) {
+        double p = 1.0, sum = 0.0;
+        for (int n = 1; n < 80; ++n) {
+            double term = 4.0 * n / (4.0 * n * n - 1.0) * p;
+            sum += term;
+            if (fabs(term) < 1e-18 * fabs(sum)) break;
+            p *= w;
+        }
+        return 0.25 / s - sum / (2.0 * kPi);
+    }
+    if (s >= 8.0) {
+        const double is = 1.0 / s;
+        double ce = 0.5 * kPi, co = 4.0 / 3.0;           // c_m for even / odd m, starting at m = 4, 5
+        double p = is * is * is, sum = 0.0;
+        for (int k = 0; k < 60; ++k) {
+            const int m = k + 4;
+            const double c = (m & 1) ? co : ce;
+            const double term = ((k & 1) ? -1.0 : 1.0) * (k + 1) * c * p;
+            sum += term;
+            if (fabs(term) < 1e-18 * fabs(sum)) break;
+            if (m & 1) co *= (double)(m - 1) / m; else ce *= (double)(m - 1) / m;
+            p *= is;
+        }
+        return sum / (4.0 * kPi);
+    }
+    double X;
+    if (w > 0.0) { const double q = sqrt(w); X = log((1.0 + q) / s) / q; }
+    else { const double q = sqrt(-w); X = acos(1.0 / s) / q; }
+    return 0.25 / s + (1.0 - (2.0 - s * s) * X) / (2.0 * kPi * w);
+}
+
+// rho_b v_r^2 = G M_b^2/(4 pi R_b^4) J3(t), t = r/R_b: the isotropic Jeans integral of eqs. B1-B2,
+//   J3 = int_t^inf dt'/(t'^3 (1+t')^3) = sum_{n>=5} (n-3)(n-4)/2 u^n/n  (u = 1/(1+t); equals rho_b x eq. B3 as corrected
+//   by reading J; the closed form cancels like t^-5 for large t, hence the series for t > 1).
+BANG_HD double jaffe_J3(double t) {                      // argument t = r/R_b (u would lose t for t << 1)
+    if (t > 1.0) {
+        const double u = 1.0 / (1.0 + t);
+        double p = u * u * u * u * u, sum = 0.0;
+        for (int n = 5; n < 400; ++n) {
+            double term = 0.5 * (n - 3) * (n - 4) * p / n;
+            sum += term;
+            if (term < 2e-18 * sum) break;
+            p *= u;
+        }
+        return sum;
+    }
+    return 1.0 / (2.0 * t * t) - 3.0 / t - 3.0 / (1.0 + t) - 1.0 / (2.0 * (1.0 + t) * (1.0 + t)) + 6.0 * log1p(1.0 / t);
+}
+
+// Scale-free l.o.s. integral for the Jaffe bulge with the same N_J-node rule as jeans_J (reading B):
+//   Sigma_b sigma_b^2 (R) = G M_b^2/(4 pi R_b^3) * 2 * JJ(s),  JJ(s) = int_0^inf J3(sqrt(s^2+z^2)) dz.
+BANG_HD double jaffe_jeans_J(double s, int NJ, const double* glx, const double* glw) {
+    const double L = sqrt(s * s + 1.0);
+    double sum = 0.0;
+    for (int k = 0; k < NJ; ++k) {
+        const double t = 0.5 * (glx[k] + 1.0), w = 0.5 * glw[k];
+        const double omt = 1.0 - t;
+        const double z = L * t * t / omt;
+        const double dzdt = L * t * (2.0 - t) / (omt * omt);
+        const double r = sqrt(s * s + z * z);
+        sum += w * dzdt * jaffe_J3(r);
+    }
+    return sum;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Modified Bessel functions I0, I1, K0, K1, exponentially scaled: I_nu(y) e^-y and K_nu(y) e^y.
 //   y <= 2 : ascending series, DLMF 10.25.2 (I_nu) and 10.31.1-2 (K_0, K_1)
 //   y  > 2 : integral representations DLMF 10.32.3  I_n(y) = (1/pi) int_0^pi e^{y cos t} cos(n t) dt  and

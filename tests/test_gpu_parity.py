@@ -217,3 +217,48 @@ def test_logl_equals_likelihood_of_the_returned_maps(bang, oracle):
     for b in range(len(th)):
         want = oracle.loglike_of_maps(maps[b], case.data, case.err, case.mask)
         assert abs(ll[b] - want) <= 1e-12 * abs(want)
+
+
+# ------------------------------------------------------------------------------------------------ Jaffe bulge (App. B)
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_jaffe_bulge_config1_grid(bang, oracle, prec):
+    # BASELINE.json config 1 with the bulge profile switched to Jaffe: fine maps, maps and logL
+    cfg = dict(W.config(1), bulge_profile=1)
+    theta = np.stack([W.theta_true(1), W.theta_true(1) * 1.01, W.theta_true(1) * 0.99])
+    theta[1, 0:2] = 0.37, -0.21                              # off-centre: the 1/R cusp is sampled asymmetrically
+    logl_o, maps_o = None, oracle.model_maps(theta, cfg)
+    data, err, mask = W.make_data(1, maps_o[0])
+    logl_o, maps_o = oracle.loglike(theta, cfg, data, err, mask, return_maps=True)
+    ctx = bang.Context(cfg, precision=prec)
+    fine = ctx.model_fine(theta[:1]).cpu().numpy()[0]
+    assert_maps(fine, oracle.model_fine(theta[0], cfg), prec, "jaffe fine")
+    ctx.set_data(data, err, mask)
+    maps = ctx.model_maps(theta).cpu().numpy()
+    ll = ctx.loglike(theta).cpu().numpy()
+    ctx.close()
+    assert_maps(maps, maps_o, prec, "jaffe maps")
+    assert_logl(ll, logl_o, maps_o, data, err, mask, prec, near=np.array([True, False, False]), what="jaffe cfg1")
+    # and the switch matters: the Hernquist maps of the same theta are different
+    ctx = bang.Context(W.config(1), precision=prec)
+    other = ctx.model_maps(theta[:1]).cpu().numpy()[0]
+    ctx.close()
+    assert np.abs(other[0] / maps_o[0, 0] - 1).max() > 1e-2
+
+
+def test_jaffe_bulge_prior_batch(bang, oracle):
+    # a seeded subset of config 2's prior-drawn batch (four components, NFW halo) with a Jaffe bulge, both precisions
+    cfg = dict(W.config(2), bulge_profile=1)
+    theta = W.theta_batch(2)
+    sub = W.parity_subset(2, theta.shape[0], 24)
+    mtrue = oracle.model_maps(W.theta_true(2), cfg)[0]
+    data, err, mask = W.make_data(2, mtrue)
+    logl_o, maps_o = oracle.loglike(theta[sub], cfg, data, err, mask, return_maps=True)
+    near = np.isin(sub, W.near_truth_slots(2, theta.shape[0]))
+    for prec in ("fp32", "fp64"):
+        ctx = bang.Context(cfg, precision=prec)
+        ctx.set_data(data, err, mask)
+        maps = ctx.model_maps(theta[sub]).cpu().numpy()
+        ll = ctx.loglike(theta[sub]).cpu().numpy()
+        ctx.close()
+        assert_maps(maps, maps_o, prec, f"jaffe cfg2 {prec}")
+        assert_logl(ll, logl_o, maps_o, data, err, mask, prec, near=near, what=f"jaffe cfg2 {prec}")

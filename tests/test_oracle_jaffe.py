@@ -107,10 +107,10 @@ def test_jaffe_dispersion_limits(oracle):
 
 def test_J3_branches_agree(oracle):
     L = oracle.lib()
-    for u in (0.499999, 0.5, 0.500001):
-        t = (1 - mp.mpf(u)) / mp.mpf(u)
-        want = 1 / (2 * t**2) - 3 / t - 3 / (1 + t) - 1 / (2 * (1 + t) ** 2) + 6 * mp.log(1 + 1 / t)
-        assert abs(L.bo_J3(u) / float(want) - 1) < 1e-13
+    for t in (0.999999, 1.0, 1.000001, 1e-9, 1e3):     # closed form (cancels ~100x at t = 1) / series
+        tt = mp.mpf(t)
+        want = mp.quad(lambda x: 1 / (x**3 * (1 + x) ** 3), [tt, 2 * tt + 1, 10 * tt + 10, mp.inf])
+        assert abs(L.bo_J3(t) / float(want) - 1) < 1e-12
 
 
 @pytest.mark.parametrize("s", S_GRID)
