@@ -112,9 +112,9 @@ class OracleLeg:
         self.theta = W.theta_batch(idx)
         mtrue = bo.model_maps(W.theta_true(idx), W.config(idx))[0]
         self.data, self.err, self.mask = W.make_data(idx, mtrue)
-        t0 = time.perf_counter()
-        self.run(np.arange(1))
-        self.t1 = time.perf_counter() - t0                   # one theta, for sizing the samples
+        self.run(np.arange(1))                               # first call: library load, thread pool
+        npilot = min(8, self.theta.shape[0])
+        self.t1 = self.run(np.arange(npilot)) / npilot       # seconds per theta, for sizing the samples
 
     def run(self, sub):
         t0 = time.perf_counter()
