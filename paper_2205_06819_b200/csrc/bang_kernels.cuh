@@ -53,10 +53,10 @@ struct ThetaC {
     int vfirst, vcells;          // per-theta v_c table: first global interval, number of intervals
     T hc, hs;                    // h cos PA, h sin PA   (h = fine cell size in kpc)
     T xp0, yp0;                  // rotated offset of cell (jcx, jcy) from the centre
-    T inv_ci2;                   // 1/cos^2 i
+    T tan2i;                     // tan^2 i = 1/cos^2 i - 1
     T invRb2, ampBb, ampIb, MLb; // bulge: s^2 = R^2 invRb2;  B_b = ampBb SigmaTilde;  B_b sigma_b^2 = ampIb J
-    T cexp[2], ampBd[2], MLd[2]; // disc j: B_d = ampBd 2^(r cexp)
-    T vk[2], q3[2];              // -sin i k_j   and   (1 - k_j^2)/3
+    T cexp[2], ampBd[2], ampSd[2]; // disc j: B_d = ampBd 2^(r cexp), Sigma_d = ampSd 2^(r cexp) = (M/L)_d B_d
+    T vkB[2], q3B[2];            // -sin i k_j ampBd_j   and   (1 - k_j^2)/3 ampBd_j: the light weights of eqs. 14, 15
     ThetaD d;
 };
 
@@ -150,7 +150,7 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, ThetaC<T
     c.xp0 = (T)(dx * cp + dy * sp);
     c.yp0 = (T)(-dx * sp + dy * cp);
     const double inv_ci2 = 1.0 / (ci * ci);
-    c.inv_ci2 = (T)inv_ci2;
+    c.tan2i = (T)((si * si) / (ci * ci));
 
     // range of radii on this theta's grid: R^2 >= dx^2+dy^2 (attained at the nearest cell); maxima at the corners
     const double floor2 = ldexp(1.0, 2 * kRFloorLog2);
@@ -191,15 +191,16 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, ThetaC<T
     }
     // discs: eq. 7-9, 11-12
     for (int j = 0; j < 2; ++j) {
-        c.cexp[j] = T(0); c.ampBd[j] = T(0); c.MLd[j] = T(1); c.vk[j] = T(0); c.q3[j] = T(0);
+        c.cexp[j] = T(0); c.ampBd[j] = T(0); c.ampSd[j] = T(0); c.vkB[j] = T(0); c.q3B[j] = T(0);
         d.Ad[j] = 0.0; d.inv2Rd[j] = 1.0;
         if (comps & (j ? C_DISC2 : C_DISC1)) {
             const double Md = exp10(th[6 + 2 * j]), Rd = th[7 + 2 * j], ML = th[13 + j], k = th[15 + j];
             c.cexp[j] = (T)(-1.4426950408889634 / Rd);
-            c.ampBd[j] = (T)(Md / (2.0 * kPi * Rd * Rd * ci) / ML * 1e-6);               // eq. 7-8
-            c.MLd[j] = (T)ML;
-            c.vk[j] = (T)(-si * k);                                                      // eq. 11
-            c.q3[j] = (T)((1.0 - k * k) / 3.0);                                          // eq. 12
+            const double aB = Md / (2.0 * kPi * Rd * Rd * ci) / ML * 1e-6;               // eq. 7-8, in Lsun/pc^2
+            c.ampBd[j] = (T)aB;
+            c.ampSd[j] = (T)(aB * ML);
+            c.vkB[j] = (T)(-si * k * aB);                                                // eq. 11 inside eq. 14
+            c.q3B[j] = (T)((1.0 - k * k) / 3.0 * aB);                                    // eq. 12 inside eq. 15
             d.Ad[j] = 2.0 * kG * Md / Rd;
             d.inv2Rd[j] = 0.5 / Rd;
         }
@@ -257,18 +258,18 @@ BANG_D void build_vc_table(const ThetaC<T>& c, const GridC& g, const FitC& fit, 
 template <typename T>
 struct CellK {
     int jcx, jcy, vfirst, vlast;
-    T hc, hs, xp0, yp0, inv_ci2;
+    T hc, hs, xp0, yp0, tan2i;
     T invRb2, ampBb, ampIb, MLb;
-    T cexp0, cexp1, ampBd0, ampBd1, MLd0, MLd1, vk0, vk1, q30, q31;
+    T cexp0, cexp1, ampBd0, ampBd1, ampSd0, ampSd1, vkB0, vkB1, q3B0, q3B1;
 };
 template <typename T>
 BANG_D CellK<T> load_cellk(const ThetaC<T>& c) {
     CellK<T> k;
     k.jcx = c.jcx; k.jcy = c.jcy; k.vfirst = c.vfirst; k.vlast = c.vcells - 1;
-    k.hc = c.hc; k.hs = c.hs; k.xp0 = c.xp0; k.yp0 = c.yp0; k.inv_ci2 = c.inv_ci2;
+    k.hc = c.hc; k.hs = c.hs; k.xp0 = c.xp0; k.yp0 = c.yp0; k.tan2i = c.tan2i;
     k.invRb2 = c.invRb2; k.ampBb = c.ampBb; k.ampIb = c.ampIb; k.MLb = c.MLb;
     k.cexp0 = c.cexp[0]; k.cexp1 = c.cexp[1]; k.ampBd0 = c.ampBd[0]; k.ampBd1 = c.ampBd[1];
-    k.MLd0 = c.MLd[0]; k.MLd1 = c.MLd[1]; k.vk0 = c.vk[0]; k.vk1 = c.vk[1]; k.q30 = c.q3[0]; k.q31 = c.q3[1];
+    k.ampSd0 = c.ampSd[0]; k.ampSd1 = c.ampSd[1]; k.vkB0 = c.vkB[0]; k.vkB1 = c.vkB[1]; k.q3B0 = c.q3B[0]; k.q3B1 = c.q3B[1];
     return k;
 }
 
@@ -289,8 +290,11 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int 
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     // (xp, yp): the cell in the galaxy frame; R on the sky (bulge), r in the disc plane
     const T floor2 = sizeof(T) == 4 ? T(0x1p-32f) : T(0x1p-32);
+    // r^2 = R^2 + y'^2 (1/cos^2 i - 1) with R^2 floored first: one FMNMX serves both radii (identical to flooring r^2
+    // itself unless 0 < R < 2^-16 kpc, where fp32 coordinates carry no information anyway; reading V)
     const T y2 = yp * yp;
-    const T r2 = fmax(fma(xp, xp, y2 * k.inv_ci2), floor2);
+    const T R2 = fmax(fma(xp, xp, y2), floor2);
+    const T r2 = fma(y2, k.tan2i, R2);
     const T rinv = fast_rsqrt(r2);
     const T r = r2 * rinv;
     const T cosphi = xp * rinv;
@@ -298,7 +302,6 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int 
     // bulge: Sigma_b (eq. 4) and Sigma_b sigma_b^2 (eq. 6) from the scale-free tables at s^2 = R^2/R_b^2
     T Bb = T(0), IbL = T(0);
     if constexpr (BULGE) {
-        const T R2 = fmax(fma(xp, xp, y2), floor2);
         T t;
         const int cell = (int)min((unsigned)(tab_cell(R2 * k.invRb2, t) - bfirst), (unsigned)blast);
         const T* p = bcoef + (size_t)cell * (2 * NC);
@@ -323,8 +326,7 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int 
     const T e1a = r * k.cexp0, e2a = r * k.cexp1;
     T shift = T(0);
     if constexpr (!BULGE) shift = SHIFT == 1 ? e1a : (SHIFT == 2 ? e2a : fmax(e1a, e2a));
-    const T Bd1 = k.ampBd0 * fast_exp2(e1a - shift);
-    const T Bd2 = k.ampBd1 * fast_exp2(e2a - shift);
+    const T E1 = fast_exp2(e1a - shift), E2 = fast_exp2(e2a - shift);     // B_d,j = ampBd_j E_j
     // v_c(r) from the per-theta table (eq. 10)
     T vc;
     {
@@ -345,11 +347,11 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int 
         vc = horner<T, D>(cv, t);
     }
     // eq. 13, 14 (with 11), 15 (with 12), 19
-    const T Btot = Bb + Bd1 + Bd2;
-    const T Stot = fma(k.MLb, Bb, fma(k.MLd0, Bd1, k.MLd1 * Bd2));         // total mass surface density (x 1e-6)
+    const T Btot = fma(k.ampBd0, E1, fma(k.ampBd1, E2, Bb));
+    const T Stot = fma(k.ampSd0, E1, fma(k.ampSd1, E2, k.MLb * Bb));       // total mass surface density (x 1e-6)
     const T invB = fast_rcp(Btot);
-    const T kB = fma(k.vk0, Bd1, k.vk1 * Bd2);
-    const T qB = fma(k.q30, Bd1, k.q31 * Bd2);
+    const T kB = fma(k.vkB0, E1, k.vkB1 * E2);                              // sum_j B_d,j (-k_j sin i)
+    const T qB = fma(k.q3B0, E1, k.q3B1 * E2);                              // sum_j B_d,j (1 - k_j^2)/3
     oV = cosphi * vc * kB * invB;
     oS = fast_sqrt(fma(vc * vc, qB, IbL) * invB);
     oLM = Btot * fast_rcp(Stot);

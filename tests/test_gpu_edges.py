@@ -66,7 +66,10 @@ def test_shapes_and_variants_match_the_oracle(bang, oracle, kw, prec, tol):
     fine = ctx.model_fine(th).cpu().numpy()
     want = oracle.model_maps(th, cfg)
     assert rel(maps, want) < tol
-    assert rel(fine, np.stack([oracle.model_fine(t, cfg) for t in th])) < tol
+    # un-convolved fine cells (a test-only intermediate, not a map pixel): theta[1] has k_1 < 0 < k_2, so the two disc
+    # terms of eq. 14 cancel and |v| falls to the fp32 noise of the terms (eps x ~150 km/s = reading P's floor of
+    # 1e-3 max|v| x 1e-4); a single fine cell may then sit at 1e-4 of that floor.  The map pixels above keep 1e-4.
+    assert rel(fine, np.stack([oracle.model_fine(t, cfg) for t in th])) < (tol if prec == "fp64" else 3 * tol)
     data, err, mask = synth_data(oracle, cfg, THETA)
     ctx.set_data(data, err, mask)
     ll = ctx.loglike(th).cpu().numpy()
