@@ -140,9 +140,10 @@ __global__ void k_univ_fit(int n_rows, FitC fit, const double* __restrict__ vals
     }
 }
 
-// data preparation (layout [ny][4][P][nxp/P]): {d, 1/e} per used pixel ({0,0} where masked or padded), C0 = sum -1/2 ln(2 pi e^2), and the number
+// data preparation (layout [ny][4][P][gmax], gmax >= nxp/P the pixel-group pitch of the launch's thread class; the
+// caller zeroes the buffer): {d, 1/e} per used pixel ({0,0} where masked or padded), C0 = sum -1/2 ln(2 pi e^2), and the number
 // of used pixels with err <= 0 or a non-finite value.  One block, deterministic reduction order.
-__global__ void k_prep_data(int nx, int ny, int nxp, int P, const double* __restrict__ data, const double* __restrict__ err,
+__global__ void k_prep_data(int nx, int ny, int nxp, int P, int gmax, const double* __restrict__ data, const double* __restrict__ err,
                             const unsigned char* __restrict__ mask, double2* __restrict__ out, double* __restrict__ scal) {
     __shared__ double sh[2][32];
     double c0 = 0.0, bad = 0.0;
@@ -162,7 +163,7 @@ __global__ void k_prep_data(int nx, int ny, int nxp, int P, const double* __rest
             }
         }
         // [py][q][i][group]: pixel px = group P + i, so that the fused kernel's load of its i-th pixel is coalesced
-        out[(((size_t)py * 4 + q) * P + px % P) * (nxp / P) + px / P] = v;
+        out[(((size_t)py * 4 + q) * P + px % P) * gmax + px / P] = v;
     }
     for (int o = 16; o > 0; o >>= 1) {
         c0 += __shfl_xor_sync(0xffffffffu, c0, o);
@@ -397,9 +398,11 @@ int bang_set_data(bang_ctx* ctx, const double* data_dev, const double* err_dev, 
     if (!data_dev || !err_dev || !mask_dev) return fail(ctx, BANG_EINVAL, "bang_set_data: null pointer");
     CU(cudaSetDevice(ctx->device));
     double2* buf = nullptr;
-    const size_t n = (size_t)ctx->g.ny * 4 * ctx->nxp;
+    const int gmax = (ctx->threads <= 128 ? 128 : (ctx->threads <= 256 ? 256 : 512)) / 4;      // lbc_threads / 4
+    const size_t n = (size_t)ctx->g.ny * 4 * ctx->P * gmax;
     CU(cudaMalloc(&buf, n * sizeof(double2)));
-    k_prep_data<<<1, 1024, 0, ctx->stream>>>(ctx->g.nx, ctx->g.ny, ctx->nxp, ctx->P, data_dev, err_dev, mask_dev, buf, ctx->scal);
+    CU(cudaMemsetAsync(buf, 0, n * sizeof(double2), ctx->stream));
+    k_prep_data<<<1, 1024, 0, ctx->stream>>>(ctx->g.nx, ctx->g.ny, ctx->nxp, ctx->P, gmax, data_dev, err_dev, mask_dev, buf, ctx->scal);
     ctx->launches += 1;
     double scal[2] = {0, 0};
     cudaError_t e = cudaGetLastError();

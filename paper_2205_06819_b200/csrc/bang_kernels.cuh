@@ -449,7 +449,8 @@ struct FusedParams {
     int B;
     int nxp;                     // data columns padded to a multiple of P
     T* maps;                     // [B][4][ny][nx]
-    const double2* data;         // [ny][4][P][nxp/P] {d, 1/e} of pixel group P + i (1/e = 0 where masked or padded)
+    const double2* data;         // [ny][4][P][GMAX] {d, 1/e} of pixel group P + i (1/e = 0 where masked or padded); GMAX =
+                                 // (thread class of the launch) / 4 >= nxp/P
     double C0;                   // sum over used pixels of -1/2 ln(2 pi e^2)
     double* logL;                // [B]
 };
@@ -495,8 +496,10 @@ BANG_D void load_run(const T* __restrict__ src, T (&f)[N]) {
 }
 
 // 1/x for the final M/L = 1/<L/M> (fn 10): MUFU.RCP (1 ulp) in fp32 mode, IEEE division in fp64 mode
-BANG_D float inv_ml(float x) { return fast_rcp(x); }
-BANG_D double inv_ml(double x) { return 1.0 / x; }
+// The argument is floored far below any physical <L/M> so that padded pixels (accumulators = 0) stay finite and drop
+// out of the chi-square through their weight 1/e = 0 without a per-pixel guard.
+BANG_D float inv_ml(float x) { return fast_rcp(fmaxf(x, 1e-30f)); }
+BANG_D double inv_ml(double x) { return 1.0 / fmax(x, 1e-300); }
 
 // MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike)
 // LBC: launch-bound class = the CTA-size bracket the kernel is compiled for, which fixes its register budget:
@@ -528,6 +531,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
     const GridC& g = p.g;
     const int tid = threadIdx.x, NT = blockDim.x;
     const int G = p.nxp / P;                         // pixel groups per map
+    constexpr int GMAX = lbc_threads(LBC) / 4;       // pitch of the data array's pixel-group axis (compile-time: immediate offsets)
     const int items = 4 * G;
     const int q = tid / G, grp = tid - q * G;        // this thread's observable and pixel group in the PSF phase
     const bool psf_thread = tid < items;
@@ -578,9 +582,9 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
                 double2 de[P];
                 if constexpr (MODE == 1) {
                     if (py >= 0) {
-                        const double2* src = p.data + ((size_t)py * 4 + q) * p.nxp + grp;
+                        const double2* src = p.data + (((py * 4 + q) * P) * GMAX + grp);
 #pragma unroll
-                        for (int i = 0; i < P; ++i) de[i] = __ldg(src + i * G);
+                        for (int i = 0; i < P; ++i) de[i] = __ldg(src + i * GMAX);
                     }
                 }
 #pragma unroll
@@ -607,7 +611,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
                             if (px < g.nx) p.maps[((size_t)b * 4 + q) * npix + (size_t)py * g.nx + px] = m;
                         } else {
                             const double z = (de[i].x - (double)m) * de[i].y;      // eq. 18, residual in fp64
-                            chi2 = (px < g.nx) ? fma(z, z, chi2) : chi2;
+                            chi2 = fma(z, z, chi2);                                // padded pixels: 1/e = 0, m finite
                         }
                     }
                 }

@@ -313,7 +313,10 @@ BANG_HD int tab_cell(float u, float& t) {
 #if defined(__CUDA_ARCH__)
     const int bits = __float_as_int(u);
     // tau = 1 + (low 19 mantissa bits) 2^-23 in [1, 1 + 2^-4);  t = 32 tau - 33, exact: one LOP3 and one FFMA
-    t = fmaf(__int_as_float((bits & 0x7FFFF) | 0x3F800000), 32.0f, -33.0f);
+    // (both masks as register operands, or ptxas splits (bits & m) | c into two LOP3 with one immediate each)
+    int tau;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(tau) : "r"(bits), "r"(0x7FFFF), "r"(0x3F800000));
+    t = fmaf(__int_as_float(tau), 32.0f, -33.0f);
 #else
     union { float f; int i; } c; c.f = u;
     const int bits = c.i;
