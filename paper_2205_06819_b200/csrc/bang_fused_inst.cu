@@ -17,7 +17,7 @@ template <typename T, int S, int NACC, int P, int MODE, int LBC>
 cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) {
     auto kern = k_fused<T, S, NACC, P, MODE, LBC>;
     if (L.threads > lbc_threads(LBC)) return cudaErrorInvalidValue;
-    const size_t smem = fused_smem_bytes<T>(S, lbc_nfb(LBC, P, S, NACC));
+    const size_t smem = fused_smem_bytes<T>(S, lbc_nfb(LBC, P, S, NACC, (int)sizeof(T)));
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;

@@ -403,7 +403,7 @@ BANG_D void eval_rows_any(const unsigned comps, const CellK<T>& k, const PolyTab
 // the rotation and the store address are shared by S cells and S independent dependency chains are in flight.
 // dst[(row * 4 + observable) * NFB + x] (NFB, the plane pitch, is a compile-time constant: immediate store offsets).  GUARD: some of the S rows lie past the grid (zero-weight tap padding): they are
 // written as zeros.
-template <typename T, int S, int NFB, bool BULGE, int SHIFT, bool GUARD>
+template <typename T, int S, int NFB, int GRP, int PADV, bool BULGE, int SHIFT, bool GUARD>
 BANG_D void eval_superrow(const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab, T* __restrict__ dst,
                           const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
     const T* __restrict__ bcoef = btab.coef;
@@ -413,7 +413,7 @@ BANG_D void eval_superrow(const CellK<T>& k, const PolyTab<T>& btab, const T* __
     for (int x = vt; x < nfx; x += NT) {
         const T a = (T)(x - k.jcx);
         const T px = fma(a, k.hc, bx), py = fma(-a, k.hs, by);
-        T* d = dst + x;
+        T* d = dst + x + (PADV ? PADV * (x / GRP) : 0);      // row_pad: GRP is a power of two whenever PADV != 0
 #pragma unroll
         for (int j = 0; j < S; ++j) {
             T vB, vV, vS, vL;
@@ -427,15 +427,15 @@ BANG_D void eval_superrow(const CellK<T>& k, const PolyTab<T>& btab, const T* __
         }
     }
 }
-template <typename T, int S, int NFB, bool GUARD>
+template <typename T, int S, int NFB, int GRP, int PADV, bool GUARD>
 BANG_D void eval_superrow_any(const unsigned comps, const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab,
                               T* __restrict__ dst, const int nfx, const int nfy, const int jy0,
                               const int vt, const int NT) {
-    if (comps & C_BULGE) eval_superrow<T, S, NFB, true, 0, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
+    if (comps & C_BULGE) eval_superrow<T, S, NFB, GRP, PADV, true, 0, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_superrow<T, S, NFB, false, 3, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else if (comps & C_DISC1) eval_superrow<T, S, NFB, false, 1, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else eval_superrow<T, S, NFB, false, 2, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
+        eval_superrow<T, S, NFB, GRP, PADV, false, 3, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else if (comps & C_DISC1) eval_superrow<T, S, NFB, GRP, PADV, false, 1, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else eval_superrow<T, S, NFB, GRP, PADV, false, 2, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
 }
 
 // ---- the fused kernel ---------------------------------------------------------------------------------------------
@@ -463,13 +463,14 @@ inline size_t fused_smem_bytes(int S, int nfb) {
 
 // N consecutive values from shared memory into registers with the widest vector loads the alignment ALIGN (bytes)
 // allows; may read up to one vector past N (the row buffer carries that slack).
-template <typename T, int N, int ALIGN>
+// GRP, PADV: the buffer holds PADV pad elements after every GRP elements (row_pad below); src points at a group start.
+template <typename T, int N, int ALIGN, int GRP, int PADV>
 BANG_D void load_run(const T* __restrict__ src, T (&f)[N]) {
     constexpr int V = ALIGN / (int)sizeof(T);
     if constexpr (V == 4) {
 #pragma unroll
         for (int i = 0; i < N; i += 4) {
-            const float4 v = *reinterpret_cast<const float4*>(src + i);
+            const float4 v = *reinterpret_cast<const float4*>(src + i + PADV * (i / GRP));
             f[i] = v.x;
             if (i + 1 < N) f[i + 1] = v.y;
             if (i + 2 < N) f[i + 2] = v.z;
@@ -485,7 +486,7 @@ BANG_D void load_run(const T* __restrict__ src, T (&f)[N]) {
     } else if constexpr (V == 2 && sizeof(T) == 8) {
 #pragma unroll
         for (int i = 0; i < N; i += 2) {
-            const double2 v = *reinterpret_cast<const double2*>(src + i);
+            const double2 v = *reinterpret_cast<const double2*>(src + i + PADV * (i / GRP));
             f[i] = v.x;
             if (i + 1 < N) f[i + 1] = v.y;
         }
@@ -509,10 +510,22 @@ constexpr int lbc_threads(int lbc) { return lbc == 0 ? 128 : (lbc == 1 ? 256 : 5
 // Row-buffer plane pitch in cells, a compile-time constant of the instantiation (so that the 4 S planes sit at immediate
 // offsets): the widest row the class can hold -- nxp <= threads P / 4 data columns -- i.e. (nxp - 1 + NACC) S cells,
 // rounded up to a multiple of 4, plus 4 cells of over-read slack for the vector loads.
-constexpr int lbc_nfb(int lbc, int P, int S, int NACC) { return ((lbc_threads(lbc) * P / 4 - 1 + NACC) * S + 3) / 4 * 4 + 4; }
+// Bank conflicts.  In the PSF phase neighbouring threads read 16-byte vectors P S elements apart.  When that stride is
+// an EVEN number of vectors (s = 4 with P = 4: 64 B), the 8 lanes of a quarter-warp fall on 2 or 4 of the 8 vector-wide
+// bank groups (ncu, config 5: 7 conflicts per load, L1 pipe 88 % busy).  One pad vector after every P S elements makes
+// the stride odd and the loads conflict-free.  row_pad = pad elements per group of P S (0 when not needed).
+constexpr int row_pad(int P, int S, int elem_bytes) {
+    const int V = 16 / elem_bytes, GRP = P * S;
+    return (GRP % V == 0 && (GRP / V) % 2 == 0) ? V : 0;
+}
+constexpr int lbc_nfb(int lbc, int P, int S, int NACC, int elem_bytes) {
+    const int cells = (lbc_threads(lbc) * P / 4 - 1 + NACC) * S;
+    const int padded = cells + row_pad(P, S, elem_bytes) * ((cells + P * S - 1) / (P * S));
+    return (padded + 3) / 4 * 4 + 4 + row_pad(P, S, elem_bytes);
+}
 constexpr int lbc_blocks(int lbc, int P, bool f64) {
     return f64 ? (lbc == 0 ? 4 : (lbc == 1 ? 2 : 1))          // fp64 mode: 128 registers in every class
-               : (lbc == 0 ? (P == 2 ? 7 : 5) : (lbc == 1 ? (P == 2 ? 3 : 2) : 1));
+               : (lbc == 0 ? (P == 2 ? 7 : 5) : (lbc == 1 ? (P == 2 ? 3 : 2) : (P == 2 ? 2 : 1)));
 }
 template <typename T, int S, int NACC, int P, int MODE, int LBC>
 __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T) == 8)) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
@@ -525,7 +538,8 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
     constexpr size_t off_tab = (sizeof(ThetaC<T>) + 15) / 16 * 16;
     T* vtab = reinterpret_cast<T*>(smem_raw + off_tab);
     T* rowbuf = vtab + (size_t)kMaxOct * (1 << TabCfg<T>::M) * NC;
-    constexpr int nfb = lbc_nfb(LBC, P, S, NACC);
+    constexpr int nfb = lbc_nfb(LBC, P, S, NACC, (int)sizeof(T));
+    constexpr int GRP = P * S, PADV = row_pad(P, S, (int)sizeof(T));
     double* red = reinterpret_cast<double*>(rowbuf + (size_t)S * 4 * nfb);
 
     const GridC& g = p.g;
@@ -537,7 +551,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
     const bool psf_thread = tid < items;
     const int nsuper = g.ny + NACC - 1;
     const size_t npix = (size_t)g.nx * g.ny;
-    const T* run_base = rowbuf + (size_t)q * nfb + grp * (P * S);
+    const T* run_base = rowbuf + (size_t)q * nfb + grp * (GRP + PADV);
 
     for (int i = tid; i < S * 4 * nfb; i += NT) rowbuf[i] = T(0);
 
@@ -569,8 +583,8 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
             // the per-theta constants are re-read from shared memory for every super-row (a handful of broadcast loads)
             // so that they do not occupy registers during the PSF phase
             const CellK<T> k = load_cellk<T>(c);
-            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, false>(g.comps, k, p.btab, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
-            else eval_superrow_any<T, S, nfb, true>(g.comps, k, p.btab, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, GRP, PADV, false>(g.comps, k, p.btab, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            else eval_superrow_any<T, S, nfb, GRP, PADV, true>(g.comps, k, p.btab, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
             vt = vt + 32 < NT ? vt + 32 : vt + 32 - NT;      // rotate the column ownership by one warp: the ragged last
                                                              // pass then falls on a different warp (scheduler) each time
             __syncthreads();
@@ -590,7 +604,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
 #pragma unroll
                 for (int j = 0; j < S; ++j) {
                     T f[RUN];
-                    load_run<T, RUN, ALIGN>(run_base + (size_t)(j * 4) * nfb, f);
+                    load_run<T, RUN, ALIGN, GRP, PADV>(run_base + (size_t)(j * 4) * nfb, f);
 #pragma unroll
                     for (int i = 0; i < P; ++i) {
                         T xp = T(0);
