@@ -504,7 +504,8 @@ BANG_D double inv_ml(double x) { return 1.0 / fmax(x, 1e-300); }
 
 // MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike)
 // LBC: launch-bound class = the CTA-size bracket the kernel is compiled for, which fixes its register budget:
-//   0: <= 128 threads, 7 (P = 2) or 5 (P = 4) CTAs per SM;  1: <= 256 threads, 3 or 2 CTAs per SM;  2: <= 512 threads.
+//   0: <= 128 threads, 7 (P = 2) or 6 (P = 4) CTAs per SM;  1: <= 256 threads, 3 or 2 CTAs per SM;  2: <= 512 threads
+//   (2 CTAs per SM with P = 2, else 1).
 // The class also fixes the row-buffer pitch (lbc_nfb), hence the shared memory per CTA.
 constexpr int lbc_threads(int lbc) { return lbc == 0 ? 128 : (lbc == 1 ? 256 : 512); }
 // Row-buffer plane pitch in cells, a compile-time constant of the instantiation (so that the 4 S planes sit at immediate
@@ -525,7 +526,7 @@ constexpr int lbc_nfb(int lbc, int P, int S, int NACC, int elem_bytes) {
 }
 constexpr int lbc_blocks(int lbc, int P, bool f64) {
     return f64 ? (lbc == 0 ? 4 : (lbc == 1 ? 2 : 1))          // fp64 mode: 128 registers in every class
-               : (lbc == 0 ? (P == 2 ? 7 : 5) : (lbc == 1 ? (P == 2 ? 3 : 2) : (P == 2 ? 2 : 1)));
+               : (lbc == 0 ? (P == 2 ? 7 : 6) : (lbc == 1 ? (P == 2 ? 3 : 2) : (P == 2 ? 2 : 1)));
 }
 template <typename T, int S, int NACC, int P, int MODE, int LBC>
 __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T) == 8)) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
