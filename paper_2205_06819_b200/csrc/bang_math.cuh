@@ -280,9 +280,10 @@ BANG_HD T nfw_mu(T x) {
 }
 template <>
 BANG_HD float nfw_mu<float>(float x) {
-    if (x < 0.125f) {
+    if (x < 0.25f) {                                  // 15 terms: x^17 < 6e-11; beyond, ln(1+x) - x/(1+x) cancels < 10x
         float sum = 0.f, p = x * x, sgn = 1.f;
-        for (int n = 2; n < 11; ++n) {
+#pragma unroll
+        for (int n = 2; n < 17; ++n) {
             sum += sgn * ((float)(n - 1) / (float)n) * p;
             p *= x;
             sgn = -sgn;
