@@ -249,6 +249,13 @@ def run_ours(args):
     roof = R.roofline(B * ncell, statistics.mean(times), cfg["supersample"], rk, prec, clocks.get("sm_mhz"), traffic)
     roof["kernel"] = "k_fused"
     roof["kernel_ms_best"] = 1e3 * min(times)
+    # measured counterparts of the derived peaks (dependency-free FFMA / MUFU / DFMA chains, bang_probe_peaks)
+    pk = ctx.probe_peaks()
+    cen = R.census(cfg["supersample"], rk, prec)
+    t_meas = B * ncell * (cen["fp64"] / pk["fp64_fma"] if prec == "fp64"
+                          else max(cen["fp32"] / pk["fp32_fma"], cen["mufu"] / pk["mufu"]))
+    roof["peaks_measured_Tinstr"] = {k: v / 1e12 for k, v in pk.items()}
+    roof["frac_of_measured_peaks"] = t_meas / statistics.mean(times)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

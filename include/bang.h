@@ -129,6 +129,13 @@ int bang_get_geometry(const bang_ctx *ctx, int *r_k, int *nfx, int *nfy);
 /* How many kernels the library has launched on this context since creation (for bench.py's gpu_launches). */
 long long bang_launch_count(const bang_ctx *ctx);
 
+/* Measurement aid, not part of the path: times dependency-free chains of FFMA,
+ * MUFU.EX2 and DFMA that fill the whole device and writes the sustained thread-level instruction rates [instr/s] to the
+ * HOST array out[3] = {fp32 FMA, MUFU, fp64 FMA}.  These are the measured counterparts of the roofline denominators
+ * that DESIGN.md derives from unit counts and clocks (128 / 16 / 64 lanes per SM per clock).  Uses the context's device
+ * and stream; synchronises.  BANG_EINVAL on NULL arguments, BANG_ECUDA on a CUDA failure. */
+int bang_probe_peaks(bang_ctx *ctx, double *out_host);
+
 void bang_destroy(bang_ctx *ctx);   /* NULL is allowed; synchronises the stream, frees everything the context owns */
 
 const char *bang_strerror(int code);               /* static string */

@@ -22,7 +22,7 @@ NTHETA = 17
 OK, EINVAL, ENOMEM, ECUDA, ENODATA = 0, -1, -2, -3, -4
 
 EXPORTS = ["bang_create", "bang_set_data", "bang_model_maps", "bang_model_fine", "bang_loglike", "bang_loglike_host",
-           "bang_model_maps_host", "bang_get_geometry", "bang_launch_count", "bang_destroy", "bang_strerror",
+           "bang_model_maps_host", "bang_get_geometry", "bang_launch_count", "bang_probe_peaks", "bang_destroy", "bang_strerror",
            "bang_last_error"]
 
 
@@ -68,6 +68,7 @@ def lib():
         L.bang_get_geometry.argtypes = [vp, C.POINTER(ip), C.POINTER(ip), C.POINTER(ip)]
         L.bang_get_geometry.restype = ip
         L.bang_launch_count.argtypes, L.bang_launch_count.restype = [vp], C.c_longlong
+        L.bang_probe_peaks.argtypes, L.bang_probe_peaks.restype = [vp, C.POINTER(C.c_double)], ip
         L.bang_destroy.argtypes, L.bang_destroy.restype = [vp], None
         L.bang_strerror.argtypes, L.bang_strerror.restype = [ip], C.c_char_p
         L.bang_last_error.argtypes, L.bang_last_error.restype = [vp], C.c_char_p
@@ -176,6 +177,12 @@ class Context:
             out = np.empty(B, dtype=np.float64)
         self._check(lib().bang_loglike_host(self._h, t.ctypes.data, B, out.ctypes.data))
         return out
+
+    def probe_peaks(self) -> dict:
+        """Measured sustained instruction rates [thread-instr/s] of dependency-free FFMA, MUFU.EX2 and DFMA chains."""
+        out = (C.c_double * 3)()
+        self._check(lib().bang_probe_peaks(self._h, out))
+        return {"fp32_fma": out[0], "mufu": out[1], "fp64_fma": out[2]}
 
     def model_maps_host(self, theta: np.ndarray) -> np.ndarray:
         t = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, NTHETA)

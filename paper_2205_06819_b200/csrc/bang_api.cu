@@ -178,6 +178,31 @@ __global__ void k_prep_data(int nx, int ny, int nxp, int P, int gmax, const doub
     }
 }
 
+// ---- peak probes (bang_probe_peaks): 8 independent chains per thread, no memory traffic --------------------------------
+template <int WHICH>
+__global__ void __launch_bounds__(256) k_probe(int iters, float seed, float* __restrict__ sink) {
+    float a[8];
+    double d[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { a[i] = seed + (float)(threadIdx.x + i) * 1e-3f; d[i] = (double)a[i]; }
+    const float m = 0.999f + seed * 1e-6f, c = 1e-3f;
+    const double md = (double)m, cd = (double)c;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (WHICH == 0) a[i] = fmaf(a[i], m, c);
+                else if (WHICH == 1) a[i] = fast_exp2(a[i]) - 1.0f;          // one MUFU.EX2 + one FADD per step
+                else d[i] = fma(d[i], md, cd);
+            }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i] + (float)d[i];
+    if (s == 12345.678f) sink[0] = s;                                     // keeps the chains alive, never true in practice
+}
+
 template <typename T>
 int build_universal(bang_ctx* ctx, const double* glx_dev, const double* glw_dev) {
     constexpr int NC = TabCfg<T>::D + 1;
@@ -274,6 +299,38 @@ int bang_get_geometry(const bang_ctx* ctx, int* r_k, int* nfx, int* nfy) {
     if (r_k) *r_k = ctx->rk;
     if (nfx) *nfx = ctx->g.nfx;
     if (nfy) *nfy = ctx->g.nfy;
+    return BANG_OK;
+}
+
+int bang_probe_peaks(bang_ctx* ctx, double* out_host) {
+    if (!ctx) return BANG_EINVAL;
+    if (!out_host) return fail(ctx, BANG_EINVAL, "bang_probe_peaks: null pointer");
+    CU(cudaSetDevice(ctx->device));
+    float* sink = nullptr;
+    CU(cudaMalloc(&sink, sizeof(float)));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+    const int grid = ctx->n_sm * 8, threads = 256, iters = 4096;
+    for (int which = 0; which < 3; ++which) {
+        const int it = which == 0 ? iters : iters / 4;
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; ++rep) {                                 // first repetition warms up
+            cudaEventRecord(e0, ctx->stream);
+            if (which == 0) k_probe<0><<<grid, threads, 0, ctx->stream>>>(it, 0.5f, sink);
+            else if (which == 1) k_probe<1><<<grid, threads, 0, ctx->stream>>>(it, 0.5f, sink);
+            else k_probe<2><<<grid, threads, 0, ctx->stream>>>(it, 0.5f, sink);
+            cudaEventRecord(e1, ctx->stream);
+            cudaError_t e = cudaEventSynchronize(e1);
+            if (e != cudaSuccess) { cudaFree(sink); return fail(ctx, BANG_ECUDA, "bang_probe_peaks: %s", cudaGetErrorString(e)); }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < best) best = ms;
+            ctx->launches += 1;
+        }
+        out_host[which] = (double)grid * threads * (double)it * 32.0 / (best * 1e-3);   // 4 x 8 chain steps per iteration
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
     return BANG_OK;
 }
 

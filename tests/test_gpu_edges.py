@@ -258,3 +258,17 @@ def test_error_codes(bang, oracle):
     with pytest.raises(bang.BangError) as ei:
         bang.Context(small_cfg(nx=4000, ny=4), precision="fp64")
     assert ei.value.code == bang.EINVAL
+
+
+def test_peak_probe_matches_the_derived_unit_counts(bang):
+    # 128 fp32 lanes, 16 MUFU results and 64 fp64 lanes per SM per clock at clocks.max.sm
+    import torch
+    ctx = bang.Context(small_cfg(), precision="fp32")
+    pk = ctx.probe_peaks()
+    ctx.close()
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    from paper_2205_06819_b200 import roofline as R
+    clk = R.sm_max_mhz() * 1e6
+    for key, lanes in (("fp32_fma", 128), ("mufu", 16), ("fp64_fma", 64)):
+        frac = pk[key] / (n_sm * lanes * clk)
+        assert 0.6 < frac < 1.08, (key, frac)
