@@ -32,6 +32,7 @@ struct bang_ctx {
     size_t cap_theta = 0, cap_out = 0;
     long long launches = 0;
     int force_ctas = 0;
+    int launch_cache[2] = {0, 0};          // per mode: resident CTAs per SM once the kernel is configured
     char err[512] = {0};
 };
 
@@ -242,7 +243,7 @@ cudaError_t dispatch_fused(const bang_ctx* c, const FusedLaunch& L, FusedInfo* i
     }
 }
 
-FusedLaunch make_launch(const bang_ctx* c, const double* theta, int B, int mode, void* maps, double* logL) {
+FusedLaunch make_launch(bang_ctx* c, const double* theta, int B, int mode, void* maps, double* logL) {
     FusedLaunch L{};
     L.g = c->g; L.fit = c->fit;
     L.btab = c->btab; L.btab_first = c->btab_first; L.btab_cells = c->btab_cells;
@@ -251,6 +252,7 @@ FusedLaunch make_launch(const bang_ctx* c, const double* theta, int B, int mode,
     L.theta = theta; L.B = B; L.P = c->P; L.nxp = c->nxp; L.mode = mode;
     L.maps = maps; L.data = c->data; L.C0 = c->C0; L.logL = logL;
     L.threads = c->threads; L.ctas = c->force_ctas; L.n_sm = c->n_sm; L.stream = c->stream;
+    L.cache = c->launch_cache;
     return L;
 }
 

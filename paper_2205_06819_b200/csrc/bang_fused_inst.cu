@@ -18,12 +18,18 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     auto kern = k_fused<T, S, NACC, P, MODE, LBC>;
     if (L.threads > lbc_threads(LBC)) return cudaErrorInvalidValue;
     const size_t smem = fused_smem_bytes<T>(S, lbc_nfb(LBC, P, S, NACC, (int)sizeof(T)));
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, L.threads, smem);
-    if (e != cudaSuccess) return e;
-    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    // the shared-memory opt-in and the occupancy query are done once per context and mode (L.cache, owned by the
+    // context): repeating them on every call costs ~10 us of host time, which a small batch notices
+    int per_sm = L.cache ? L.cache[L.mode] : 0;
+    cudaError_t e;
+    if (per_sm < 1) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, L.threads, smem);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+        if (L.cache && !query_only) L.cache[L.mode] = per_sm;
+    }
     int ctas = L.ctas > 0 ? L.ctas : per_sm * L.n_sm;
     if (ctas > L.B) ctas = L.B;
     if (info) {

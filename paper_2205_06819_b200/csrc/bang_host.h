@@ -21,6 +21,7 @@ struct FusedLaunch {
     double* logL;
     int threads, ctas;           // launch shape (ctas = 0: let the launcher size a persistent grid)
     int n_sm;
+    int* cache;                  // [2] resident CTAs per SM of the mode's kernel once configured (0 = not yet), or NULL
     cudaStream_t stream;
 };
 
