@@ -294,7 +294,7 @@ def run_ours(args):
         line["sweep"] = sweep
     if rank == 0:
         print(json.dumps(line))
-    if world > 1:
+    if torch.distributed.is_available() and torch.distributed.is_initialized():
         torch.distributed.destroy_process_group()
 
 

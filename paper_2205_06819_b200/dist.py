@@ -25,13 +25,21 @@ def shard(theta: np.ndarray, rank: int, world: int) -> np.ndarray:
     return theta[lo:hi]
 
 
+def _reduce_device(device):
+    """Where a scalar to be all-reduced must live: NCCL reduces CUDA tensors only, gloo takes CPU tensors."""
+    import torch.distributed as dist
+    if device is not None:
+        return device
+    return "cuda" if dist.get_backend() == "nccl" else "cpu"
+
+
 def max_over_ranks(value: float, device=None) -> float:
     """max of a per-rank scalar (device time); identity when torch.distributed is not initialised."""
     import torch
     import torch.distributed as dist
     if not (dist.is_available() and dist.is_initialized()):
         return float(value)
-    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    t = torch.tensor([value], dtype=torch.float64, device=_reduce_device(device))
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
 
@@ -41,7 +49,7 @@ def sum_over_ranks(value: float, device=None) -> float:
     import torch.distributed as dist
     if not (dist.is_available() and dist.is_initialized()):
         return float(value)
-    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    t = torch.tensor([value], dtype=torch.float64, device=_reduce_device(device))
     dist.all_reduce(t, op=dist.ReduceOp.SUM)
     return float(t.item())
 
