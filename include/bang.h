@@ -136,6 +136,17 @@ long long bang_launch_count(const bang_ctx *ctx);
  * and stream; synchronises.  BANG_EINVAL on NULL arguments, BANG_ECUDA on a CUDA failure. */
 int bang_probe_peaks(bang_ctx *ctx, double *out_host);
 
+/* Pre-step: resolved M/L maps from two photometric bands through a colour-M/L relation,
+ * eq. 20 with the error model of App. C:
+ *   log10 (M/L) = a + b (m_beta - m_gamma),   d log10(M/L) = sqrt(b^2 (dm_beta^2 + dm_gamma^2) + sigma_alpha^2),
+ *   d(M/L) = ln 10 (M/L) d log10(M/L).   (The paper's test case: a = -0.70, b = 0.89, sigma_alpha = 0.07.)
+ * All arrays are DEVICE pointers of n doubles (magnitudes and their errors in, M/L and its error out; out may alias
+ * nothing).  Non-finite inputs give non-finite outputs for that pixel.  No context: runs on `device`, enqueued on
+ * `cuda_stream` (asynchronous).  BANG_EINVAL on NULL pointers, BANG_ECUDA on a CUDA failure. */
+int bang_ml_from_colour(const double *m_beta_dev, const double *m_gamma_dev, const double *dm_beta_dev,
+                        const double *dm_gamma_dev, long long n, double a, double b, double sigma_alpha,
+                        double *ml_dev, double *ml_err_dev, int device, void *cuda_stream);
+
 void bang_destroy(bang_ctx *ctx);   /* NULL is allowed; synchronises the stream, frees everything the context owns */
 
 const char *bang_strerror(int code);               /* static string */

@@ -561,6 +561,19 @@ int bo_model_maps(const double *theta, int B, int nx, int ny, double pix, int s,
     return 0;
 }
 
+// eq. 20 with the error model of App. C: log10 (M/L)_alpha = a + b (m_beta - m_gamma);
+// its uncertainty propagates the magnitude errors and adds the scatter sigma_alpha of the relation in quadrature:
+// d log10(M/L) = sqrt(b^2 (dm_beta^2 + dm_gamma^2) + sigma_alpha^2);  to first order d(M/L) = ln 10 (M/L) d log10(M/L).
+void bo_ml_from_colour(const double *m_beta, const double *m_gamma, const double *dm_beta, const double *dm_gamma,
+                       long n, double a, double b, double sigma_alpha, double *ml, double *ml_err) {
+    for (long i = 0; i < n; ++i) {
+        double logml = a + b * (m_beta[i] - m_gamma[i]);
+        double dlog = std::sqrt(b * b * (dm_beta[i] * dm_beta[i] + dm_gamma[i] * dm_gamma[i]) + sigma_alpha * sigma_alpha);
+        ml[i] = std::pow(10.0, logml);
+        ml_err[i] = std::log(10.0) * ml[i] * dlog;
+    }
+}
+
 // step 11, eq. 18 (reading L): Gaussian log-likelihood of given model maps.
 double bo_loglike_of_maps(const double *maps, const double *data, const double *err, const unsigned char *mask,
                           int nx, int ny) {

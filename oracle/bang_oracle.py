@@ -62,6 +62,8 @@ def lib():
         L.bo_convolve_rebin.argtypes, L.bo_convolve_rebin.restype = [_dp, _i, _i, _i, _d, _d, _dp], _i
         L.bo_model_maps.argtypes, L.bo_model_maps.restype = [_dp, _i] + cfg + [_dp], _i
         L.bo_loglike_of_maps.argtypes, L.bo_loglike_of_maps.restype = [_dp, _dp, _dp, _bp, _i, _i], _d
+        L.bo_ml_from_colour.argtypes = [_dp, _dp, _dp, _dp, C.c_long, _d, _d, _d, _dp, _dp]
+        L.bo_ml_from_colour.restype = None
         L.bo_loglike.argtypes = [_dp, _i] + cfg + [_dp, _dp, _bp, _dp, C.c_void_p]
         L.bo_loglike.restype = _i
         _lib = L
@@ -157,3 +159,11 @@ def loglike(theta, cfg, data, err, mask, return_maps: bool = False):
     if rc != 0:
         raise ValueError(f"bo_loglike rc={rc}")
     return (out, maps) if return_maps else out
+
+
+def ml_from_colour(m_beta, m_gamma, dm_beta, dm_gamma, a=-0.70, b=0.89, sigma_alpha=0.07):
+    """eq. 20 with App. C's error model (defaults: the paper's g-i / i-band constants)."""
+    arrs = [np.ascontiguousarray(x, dtype=np.float64) for x in (m_beta, m_gamma, dm_beta, dm_gamma)]
+    ml, err = np.empty_like(arrs[0]), np.empty_like(arrs[0])
+    lib().bo_ml_from_colour(*[x.ravel() for x in arrs], arrs[0].size, a, b, sigma_alpha, ml.reshape(-1), err.reshape(-1))
+    return ml, err

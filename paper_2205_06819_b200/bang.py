@@ -22,7 +22,7 @@ NTHETA = 17
 OK, EINVAL, ENOMEM, ECUDA, ENODATA = 0, -1, -2, -3, -4
 
 EXPORTS = ["bang_create", "bang_set_data", "bang_model_maps", "bang_model_fine", "bang_loglike", "bang_loglike_host",
-           "bang_model_maps_host", "bang_get_geometry", "bang_launch_count", "bang_probe_peaks", "bang_destroy", "bang_strerror",
+           "bang_model_maps_host", "bang_get_geometry", "bang_launch_count", "bang_probe_peaks", "bang_ml_from_colour", "bang_destroy", "bang_strerror",
            "bang_last_error"]
 
 
@@ -69,6 +69,8 @@ def lib():
         L.bang_get_geometry.restype = ip
         L.bang_launch_count.argtypes, L.bang_launch_count.restype = [vp], C.c_longlong
         L.bang_probe_peaks.argtypes, L.bang_probe_peaks.restype = [vp, C.POINTER(C.c_double)], ip
+        L.bang_ml_from_colour.argtypes = [vp, vp, vp, vp, C.c_longlong, dp, dp, dp, vp, vp, ip, vp]
+        L.bang_ml_from_colour.restype = ip
         L.bang_destroy.argtypes, L.bang_destroy.restype = [vp], None
         L.bang_strerror.argtypes, L.bang_strerror.restype = [ip], C.c_char_p
         L.bang_last_error.argtypes, L.bang_last_error.restype = [vp], C.c_char_p
@@ -190,3 +192,20 @@ class Context:
         out = np.empty((B, 4, self.ny, self.nx), dtype=self.np_dtype)
         self._check(lib().bang_model_maps_host(self._h, t.ctypes.data, B, out.ctypes.data))
         return out
+
+
+def ml_from_colour(m_beta, m_gamma, dm_beta, dm_gamma, a=-0.70, b=0.89, sigma_alpha=0.07, device=0):
+    """eq. 20 with App. C's error model on the device: magnitude maps (and errors) -> (M/L, its error), float64 tensors."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bang.ml_from_colour needs a CUDA device (there is no CPU fallback)")
+    dev = torch.device("cuda", device)
+    x = [torch.as_tensor(v, dtype=torch.float64, device=dev).contiguous() for v in (m_beta, m_gamma, dm_beta, dm_gamma)]
+    assert all(t.shape == x[0].shape for t in x)
+    ml, err = torch.empty_like(x[0]), torch.empty_like(x[0])
+    rc = lib().bang_ml_from_colour(x[0].data_ptr(), x[1].data_ptr(), x[2].data_ptr(), x[3].data_ptr(), x[0].numel(),
+                                   float(a), float(b), float(sigma_alpha), ml.data_ptr(), err.data_ptr(), device,
+                                   C.c_void_p(torch.cuda.current_stream(dev).cuda_stream))
+    if rc != OK:
+        raise BangError(rc, lib().bang_strerror(rc).decode())
+    return ml, err
