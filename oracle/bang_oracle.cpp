@@ -331,6 +331,7 @@ struct Setup {
     unsigned comps;
     int halo_profile;                  // 0 Hernquist (paper), 1 NFW (reading H)
     int bulge_profile;                 // 0 Hernquist (paper default), 1 Jaffe (App. B)
+    int psf_weighting;                 // 0: the paper's eq. 21 on B, v, sigma, <L/M> (reading G); 1: flux-weighted moments (reading G')
     std::vector<double> taps, glx, glw;
 };
 
@@ -351,15 +352,16 @@ void psf_taps(double sigma_pix, int s, double trunc, std::vector<double> &g) {
     for (double &v : g) v /= sum;
 }
 
-// profiles: bits 0-7 halo profile, bits 8-15 bulge profile
+// profiles: bits 0-7 halo profile, bits 8-15 bulge profile, bits 16-23 PSF weighting
 bool make_setup(Setup &S, int nx, int ny, double pix, int s, double dist_mpc, double sigma_pix,
                 double trunc, unsigned comps, int profiles, int NJ) {
     const int halo_profile = profiles & 0xff, bulge_profile = (profiles >> 8) & 0xff;
-    if (halo_profile > 1 || bulge_profile > 1) return false;
+    const int psf_weighting = (profiles >> 16) & 0xff;
+    if (halo_profile > 1 || bulge_profile > 1 || psf_weighting > 1) return false;
     if (nx < 1 || ny < 1 || s < 1 || !(pix > 0) || !(dist_mpc > 0) || sigma_pix < 0 || NJ < 1) return false;
     if (!(comps & (C_BULGE | C_DISC1 | C_DISC2))) return false;
     S.nx = nx; S.ny = ny; S.s = s; S.pix = pix; S.kappa = dist_mpc * kArcsecKpcPerMpc;
-    S.comps = comps; S.halo_profile = halo_profile; S.bulge_profile = bulge_profile; S.NJ = NJ;
+    S.comps = comps; S.halo_profile = halo_profile; S.bulge_profile = bulge_profile; S.psf_weighting = psf_weighting; S.NJ = NJ;
     psf_taps(sigma_pix, s, trunc, S.taps);
     S.rk = (int(S.taps.size()) - 1) / 2;
     S.nfx = nx * s + 2 * S.rk; S.nfy = ny * s + 2 * S.rk;
@@ -420,6 +422,15 @@ void fine_cell(const Setup &S, const Theta &t, int Jx, int Jy, double out[4]) {
     out[1] = (Bd[0] * vd[0] + Bd[1] * vd[1]) / Btot;
     out[2] = std::sqrt((IbL + Bd[0] * sd2[0] + Bd[1] * sd2[1]) / Btot);
     out[3] = Btot / ((Sb + Sd[0] + Sd[1]) * 1e-6);
+    if (S.psf_weighting == 1) {
+        // reading G': what the beam averages is light, not velocity -- the fields handed to
+        // the PSF are the zeroth, first and second velocity moments of the light and the mass surface density:
+        // B, B v_los, B (sigma_los^2 + v_los^2), Sigma_tot [x 1e-6], with v_los, sigma_los of eqs. 14-15 above
+        const double v = out[1], sg = out[2];
+        out[1] = Btot * v;
+        out[2] = Btot * (sg * sg + v * v);
+        out[3] = (Sb + Sd[0] + Sd[1]) * 1e-6;
+    }
 }
 
 // fine maps [4][nfy][nfx], un-convolved
@@ -459,8 +470,19 @@ void convolve_rebin(const Setup &S, const double *fine, double *maps) {
                 for (int by = 0; by < S.s; ++by)
                     for (int bx = 0; bx < S.s; ++bx) a += txy[(size_t)(py * S.s + by) * nix + (px * S.s + bx)];
                 a /= (double)(S.s * S.s);
-                maps[((size_t)q * S.ny + py) * S.nx + px] = (q == 3) ? 1.0 / a : a;
+                maps[((size_t)q * S.ny + py) * S.nx + px] = (q == 3 && S.psf_weighting == 0) ? 1.0 / a : a;
             }
+    }
+    if (S.psf_weighting == 1) {
+        // reading G': observables from the beam-averaged moments M0..M3 of a pixel:
+        // B = M0, v = M1/M0, sigma = sqrt(M2/M0 - v^2) (never negative analytically; floored at 0), M/L = M3/M0
+        const size_t np = (size_t)S.nx * S.ny;
+        for (size_t i = 0; i < np; ++i) {
+            const double M0 = maps[i], v = maps[np + i] / M0;
+            maps[np + i] = v;
+            maps[2 * np + i] = std::sqrt(std::max(maps[2 * np + i] / M0 - v * v, 0.0));
+            maps[3 * np + i] = maps[3 * np + i] / M0;
+        }
     }
 }
 
@@ -544,9 +566,10 @@ int bo_model_fine(const double *theta, int nx, int ny, double pix, int s, double
 }
 
 // steps 9-10 alone on caller-supplied fine maps (pin: brute-force 2-D sums, flux conservation)
-int bo_convolve_rebin(const double *fine, int nx, int ny, int s, double sigma_pix, double trunc, double *maps) {
+int bo_convolve_rebin(const double *fine, int nx, int ny, int s, double sigma_pix, double trunc, int psf_weighting,
+                      double *maps) {
     Setup S;
-    if (!make_setup(S, nx, ny, 1.0, s, 1.0, sigma_pix, trunc, C_DISC1, 0, 1)) return -1;
+    if (!make_setup(S, nx, ny, 1.0, s, 1.0, sigma_pix, trunc, C_DISC1, psf_weighting << 16, 1)) return -1;
     convolve_rebin(S, fine, maps);
     return 0;
 }

@@ -59,7 +59,7 @@ def lib():
         L.bo_psf_taps.argtypes, L.bo_psf_taps.restype = [_d, _i, _d, _dp], _i
         cfg = [_i, _i, _d, _i, _d, _d, _d, _u, _i, _i]   # nx ny pix s dist sigma trunc comps profiles NJ
         L.bo_model_fine.argtypes, L.bo_model_fine.restype = [_dp] + cfg + [_dp], _i
-        L.bo_convolve_rebin.argtypes, L.bo_convolve_rebin.restype = [_dp, _i, _i, _i, _d, _d, _dp], _i
+        L.bo_convolve_rebin.argtypes, L.bo_convolve_rebin.restype = [_dp, _i, _i, _i, _d, _d, _i, _dp], _i
         L.bo_model_maps.argtypes, L.bo_model_maps.restype = [_dp, _i] + cfg + [_dp], _i
         L.bo_loglike_of_maps.argtypes, L.bo_loglike_of_maps.restype = [_dp, _dp, _dp, _bp, _i, _i], _d
         L.bo_ml_from_colour.argtypes = [_dp, _dp, _dp, _dp, C.c_long, _d, _d, _d, _dp, _dp]
@@ -80,10 +80,10 @@ def get_threads() -> int:
 
 def _cfg(cfg):
     """cfg: dict with nx ny pix_arcsec supersample dist_mpc sigma_pix trunc_nsigma components halo_profile
-    [bulge_profile] jeans_nodes.  The two profile switches travel in one int: halo | bulge << 8."""
+    [bulge_profile] jeans_nodes.  The switches travel in one int: halo | bulge << 8 | psf_weighting << 16."""
     return (int(cfg["nx"]), int(cfg["ny"]), float(cfg["pix_arcsec"]), int(cfg["supersample"]),
             float(cfg["dist_mpc"]), float(cfg["sigma_pix"]), float(cfg.get("trunc_nsigma", 3.0)),
-            int(cfg["components"]), int(cfg.get("halo_profile", 0)) | (int(cfg.get("bulge_profile", 0)) << 8),
+            int(cfg["components"]), int(cfg.get("halo_profile", 0)) | (int(cfg.get("bulge_profile", 0)) << 8) | (int(cfg.get("psf_weighting", 0)) << 16),
             int(cfg["jeans_nodes"]))
 
 
@@ -118,10 +118,10 @@ def model_fine(theta, cfg) -> np.ndarray:
     return out
 
 
-def convolve_rebin(fine, nx, ny, s, sigma_pix, trunc=3.0) -> np.ndarray:
+def convolve_rebin(fine, nx, ny, s, sigma_pix, trunc=3.0, psf_weighting=0) -> np.ndarray:
     fine = np.ascontiguousarray(fine, dtype=np.float64)
     out = np.zeros((4, ny, nx))
-    rc = lib().bo_convolve_rebin(fine, nx, ny, s, sigma_pix, trunc, out)
+    rc = lib().bo_convolve_rebin(fine, nx, ny, s, sigma_pix, trunc, int(psf_weighting), out)
     if rc != 0:
         raise ValueError(f"bo_convolve_rebin rc={rc}")
     return out
