@@ -60,6 +60,11 @@ extern "C" {
                                     integral of eq. B1 x B3 (B3 as corrected by reading J), which eq. B5 pins */
 #define BANG_HALO_HERNQUIST  0   /* the paper's halo: eq. 2 with (M_h, R_h) */
 #define BANG_HALO_NFW        1   /* BASELINE.json configs 2-5: (log10 M200, c), H0 = 70 km/s/Mpc (reading H) */
+#define BANG_PSF_FIELDS 0        /* the paper: eq. 21 applied to B, v_los, sigma_los, <L/M> separately (reading G) */
+#define BANG_PSF_FLUX   1        /* variant (reading G'): PSF + rebin applied to the light moments B, B v, B (sigma^2 + v^2)
+                                    and to the mass surface density; v = M1/M0, sigma^2 = M2/M0 - v^2, M/L = M3/M0.
+                                    bang_model_fine then returns those four moment fields.  A side variant, run UNFUSED
+                                    (moment fields through HBM scratch, several kernels per call), not the tuned path */
 #define BANG_FP32 0              /* fp32 model arithmetic; residuals and logL accumulation in fp64 */
 #define BANG_FP64 1              /* everything in fp64 */
 
@@ -83,6 +88,7 @@ typedef struct {
     int halo_profile;      /* BANG_HALO_HERNQUIST or BANG_HALO_NFW */
     int jeans_nodes;       /* N_J >= 1: nodes of the Gauss-Legendre rule for the bulge Jeans l.o.s. integral (reading B) */
     int precision;         /* BANG_FP32 or BANG_FP64 */
+    int psf_weighting;     /* BANG_PSF_FIELDS (the paper) or BANG_PSF_FLUX */
 } bang_model;
 
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (NULL = the legacy default stream) on

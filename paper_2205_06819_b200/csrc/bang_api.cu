@@ -9,6 +9,7 @@
 
 #include "../../include/bang.h"
 #include "bang_host.h"
+#include "bang_moments.cuh"
 
 using namespace bang;
 
@@ -32,7 +33,10 @@ struct bang_ctx {
     size_t cap_theta = 0, cap_out = 0;
     long long launches = 0;
     int force_ctas = 0;
-    int launch_cache[2] = {0, 0};          // per mode: resident CTAs per SM once the kernel is configured
+    int launch_cache[2] = {0, 0};
+    // flux-weighted PSF variant (unfused): composite taps on the device, scratch for the moment fields of a chunk of theta
+    double* W_dev = nullptr; void* fx_fine = nullptr; int* fx_valid = nullptr; double* fx_chi2 = nullptr;
+    int fx_chunk = 0; size_t fx_chi2_cap = 0;          // per mode: resident CTAs per SM once the kernel is configured
     char err[512] = {0};
 };
 
@@ -290,6 +294,51 @@ int ensure_staging(bang_ctx* ctx, int B, size_t out_bytes) {
     return BANG_OK;
 }
 
+// BANG_PSF_FLUX: k_fine (moment fields of a chunk of theta -> HBM scratch) + k_psf_moments (+ k_moments_reduce)
+template <typename T>
+int run_flux(bang_ctx* ctx, const double* theta_dev, int B, int mode, void* maps_dev, double* logL_dev) {
+    const GridC& g = ctx->g;
+    const size_t plane4 = (size_t)4 * g.nfx * g.nfy * sizeof(T);
+    const int ntap = 2 * ctx->rk + g.s;
+    if (!ctx->W_dev) {
+        CU(cudaMalloc(&ctx->W_dev, ntap * sizeof(double)));
+        CU(cudaMemcpyAsync(ctx->W_dev, ctx->W.data(), ntap * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));                      // ctx->W is pageable host memory
+    }
+    if (!ctx->fx_fine) {                                              // scratch: at most 256 MiB of moment fields
+        ctx->fx_chunk = (int)std::max<size_t>(1, std::min<size_t>(4096, ((size_t)256 << 20) / plane4));
+        CU(cudaMalloc(&ctx->fx_fine, (size_t)ctx->fx_chunk * plane4));
+        CU(cudaMalloc(&ctx->fx_valid, (size_t)ctx->fx_chunk * sizeof(int)));
+    }
+    if (mode == 1 && (size_t)B * g.ny > ctx->fx_chi2_cap) {
+        cudaFree(ctx->fx_chi2); ctx->fx_chi2 = nullptr; ctx->fx_chi2_cap = 0;
+        CU(cudaMalloc(&ctx->fx_chi2, (size_t)B * g.ny * sizeof(double)));
+        ctx->fx_chi2_cap = (size_t)B * g.ny;
+    }
+    const size_t smem = fused_smem_bytes<T>(0, 0);
+    CU(cudaFuncSetAttribute(k_fine<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int gmax = (ctx->threads <= 128 ? 128 : (ctx->threads <= 256 ? 256 : 512)) / 4;
+    for (int b0 = 0; b0 < B; b0 += ctx->fx_chunk) {
+        const int Bc = std::min(ctx->fx_chunk, B - b0);
+        const double* th = theta_dev + (size_t)b0 * kNTheta;
+        k_theta_valid<T><<<(Bc + 127) / 128, 128, 0, ctx->stream>>>(th, Bc, g, ctx->fx_valid);
+        FineParams<T> fp{g, ctx->fit, PolyTab<T>{static_cast<const T*>(ctx->btab), ctx->btab_first, ctx->btab_cells},
+                         PolyTab<T>{static_cast<const T*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells}, th, Bc,
+                         static_cast<T*>(ctx->fx_fine)};
+        k_fine<T><<<std::min(Bc, 8 * ctx->n_sm), 256, smem, ctx->stream>>>(fp);
+        MomentsParams<T> mp{g, ntap, ctx->W_dev, static_cast<const T*>(ctx->fx_fine), Bc, b0, ctx->fx_valid,
+                            static_cast<T*>(maps_dev), ctx->data, ctx->P, gmax, ctx->fx_chi2, mode};
+        k_psf_moments<T><<<Bc * g.ny, 128, 0, ctx->stream>>>(mp);
+        ctx->launches += 3;
+        if (mode == 1) {
+            k_moments_reduce<<<(Bc + 127) / 128, 128, 0, ctx->stream>>>(ctx->fx_chi2, ctx->fx_valid, Bc, b0, g.ny, ctx->C0, logL_dev);
+            ctx->launches += 1;
+        }
+        CU(cudaGetLastError());
+    }
+    return BANG_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -371,6 +420,7 @@ void bang_destroy(bang_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     cudaFree(ctx->btab); cudaFree(ctx->Ftab); cudaFree(ctx->data); cudaFree(ctx->scal);
     cudaFree(ctx->d_theta); cudaFree(ctx->d_out);
+    cudaFree(ctx->W_dev); cudaFree(ctx->fx_fine); cudaFree(ctx->fx_valid); cudaFree(ctx->fx_chi2);
     if (ctx->h_theta) cudaFreeHost(ctx->h_theta);
     if (ctx->h_out) cudaFreeHost(ctx->h_out);
     delete ctx;
@@ -391,6 +441,8 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     if (model->halo_profile != BANG_HALO_HERNQUIST && model->halo_profile != BANG_HALO_NFW) return BANG_EINVAL;
     if (model->jeans_nodes < 1 || model->jeans_nodes > 4096) return BANG_EINVAL;
     if (model->precision != BANG_FP32 && model->precision != BANG_FP64) return BANG_EINVAL;
+    if (model->psf_weighting != BANG_PSF_FIELDS && model->psf_weighting != BANG_PSF_FLUX) return BANG_EINVAL;
+    if (model->psf_weighting != BANG_PSF_FIELDS && model->psf_weighting != BANG_PSF_FLUX) return BANG_EINVAL;
 
     const int s = grid->supersample;
     const int rk = (int)std::ceil(psf->trunc_nsigma * psf->sigma_pix * s - 1e-9);
@@ -418,6 +470,8 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     g.spx = s / grid->pix_arcsec;
     g.h = grid->pix_arcsec * grid->dist_mpc * kKpcPerArcsecPerMpc / s;
     g.comps = model->components; g.halo_profile = model->halo_profile; g.bulge_profile = model->bulge_profile;
+    g.flux = model->psf_weighting;
+    g.flux = model->psf_weighting;
 
     // eq. 21 on the fine grid, separable (reading F): g[m] = exp(-m^2/(2 sigma_f^2)), normalised;
     // composed with the s-cell box of the rebin: W[t] = (1/s) sum_{b<s} g[t - b], t = 0 .. 2 r_k + s - 1.
@@ -511,6 +565,9 @@ int bang_model_maps(bang_ctx* ctx, const double* theta_dev, int B, void* maps_de
     if (B < 0 || (B > 0 && (!theta_dev || !maps_dev))) return fail(ctx, BANG_EINVAL, "bang_model_maps: bad arguments");
     if (B == 0) return BANG_OK;
     CU(cudaSetDevice(ctx->device));
+    if (ctx->model.psf_weighting == BANG_PSF_FLUX)
+        return ctx->model.precision == BANG_FP64 ? run_flux<double>(ctx, theta_dev, B, 0, maps_dev, nullptr)
+                                                 : run_flux<float>(ctx, theta_dev, B, 0, maps_dev, nullptr);
     FusedLaunch L = make_launch(ctx, theta_dev, B, 0, maps_dev, nullptr);
     CU(dispatch_fused(ctx, L, nullptr, false));
     ctx->launches += 1;
@@ -523,6 +580,9 @@ int bang_loglike(bang_ctx* ctx, const double* theta_dev, int B, double* logL_dev
     if (!ctx->has_data) return fail(ctx, BANG_ENODATA, "bang_loglike: no data loaded");
     if (B == 0) return BANG_OK;
     CU(cudaSetDevice(ctx->device));
+    if (ctx->model.psf_weighting == BANG_PSF_FLUX)
+        return ctx->model.precision == BANG_FP64 ? run_flux<double>(ctx, theta_dev, B, 1, nullptr, logL_dev)
+                                                 : run_flux<float>(ctx, theta_dev, B, 1, nullptr, logL_dev);
     FusedLaunch L = make_launch(ctx, theta_dev, B, 1, nullptr, logL_dev);
     CU(dispatch_fused(ctx, L, nullptr, false));
     ctx->launches += 1;

@@ -70,6 +70,8 @@ struct GridC {
     unsigned comps;
     int halo_profile;            // 0 Hernquist (paper), 1 NFW (reading H)
     int bulge_profile;           // 0 Hernquist (paper default), 1 Jaffe (App. B)
+    int flux;                    // 1: flux-weighted PSF variant (reading G'): k_fine writes the light moments; the fused
+                                 // kernel is not used (bang_api.cu runs k_fine + k_psf_moments instead)
 };
 
 struct FitC {                    // Chebyshev-node fit of degree D: nodes t_k and the inverse Vandermonde matrix
@@ -338,7 +340,7 @@ BANG_D void rotate_cell(const CellK<T>& k, const T a, const T b, T& xp, T& yp) {
 // a2 + a3: one fine cell at (xp, yp) in the galaxy frame -> B_tot, v_los, sigma_los, <L/M>   (eqs. 4-15, 19).  BULGE: the model has a bulge; SHIFT = 0/1/2/3: without a bulge
 // the disc exponentials are scaled by disc 1 (1), disc 2 (2) or the larger of the two (3) so that the ratios below
 // survive fp32 underflow far outside small discs.
-template <typename T, bool BULGE, int SHIFT>
+template <typename T, bool BULGE, int SHIFT, bool FLUX = false>
 BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int bfirst, const int blast,
                       const T* __restrict__ vtab, const T xp, const T yp, T& oB, T& oV, T& oS, T& oLM) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
@@ -410,6 +412,14 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int 
     oS = fast_sqrt(fma(vc * vc, qB, IbL) * invB);
     oLM = Btot * fast_rcp(Stot);
     oB = BULGE ? Btot : Btot * fast_exp2(shift);
+    if constexpr (FLUX) {
+        // reading G': the PSF acts on the light moments B, B v, B (sigma^2 + v^2) and on the mass surface density
+        // B / <L/M>; formed from the finished observables (k_fine only: the fused kernel never instantiates this)
+        const T v = oV;
+        oV = oB * v;
+        oS = oB * fma(oS, oS, v * v);
+        oLM = oB * fast_rcp(oLM);
+    }
 }
 
 // a2 + a3 over a run of whole fine rows: cells i = tid, tid + NT, ... of the n_rows x nfx block that starts at fine row
@@ -421,7 +431,7 @@ BANG_D EvalWalk make_walk(const int tid, const int NT, const int nfx) {
     w.step_j = NT / nfx; w.step_x = NT - w.step_j * nfx;
     return w;
 }
-template <typename T, bool BULGE, int SHIFT>
+template <typename T, bool BULGE, int SHIFT, bool FLUX>
 BANG_D void eval_rows(const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab, T* __restrict__ dst,
                       const size_t row_pitch, const size_t obs_stride, const int nfx, const int jy0, const int n_rows,
                       const EvalWalk& w, const int NT) {
@@ -434,22 +444,29 @@ BANG_D void eval_rows(const CellK<T>& k, const PolyTab<T>& btab, const T* __rest
     for (int i = tid; i < n; i += NT) {
         T vB, vV, vS, vL, xp, yp;
         rotate_cell<T>(k, (T)(x - k.jcx), (T)(jy0 + j - k.jcy), xp, yp);
-        eval_cell<T, BULGE, SHIFT>(k, bcoef, bfirst, blast, vtab, xp, yp, vB, vV, vS, vL);
+        eval_cell<T, BULGE, SHIFT, FLUX>(k, bcoef, bfirst, blast, vtab, xp, yp, vB, vV, vS, vL);
         T* d = dst + (size_t)j * row_pitch + x;
         d[0] = vB; d[obs_stride] = vV; d[2 * obs_stride] = vS; d[3 * obs_stride] = vL;
         x += step_x; j += step_j;
         if (x >= nfx) { x -= nfx; ++j; }
     }
 }
-template <typename T>
-BANG_D void eval_rows_any(const unsigned comps, const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab,
-                          T* __restrict__ dst, const size_t row_pitch, const size_t obs_stride, const int nfx,
-                          const int jy0, const int n_rows, const EvalWalk& w, const int NT) {
-    if (comps & C_BULGE) eval_rows<T, true, 0>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+template <typename T, bool FLUX>
+BANG_D void eval_rows_comps(const unsigned comps, const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab,
+                            T* __restrict__ dst, const size_t row_pitch, const size_t obs_stride, const int nfx,
+                            const int jy0, const int n_rows, const EvalWalk& w, const int NT) {
+    if (comps & C_BULGE) eval_rows<T, true, 0, FLUX>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_rows<T, false, 3>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
-    else if (comps & C_DISC1) eval_rows<T, false, 1>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
-    else eval_rows<T, false, 2>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+        eval_rows<T, false, 3, FLUX>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else if (comps & C_DISC1) eval_rows<T, false, 1, FLUX>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else eval_rows<T, false, 2, FLUX>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+}
+template <typename T>
+BANG_D void eval_rows_any(const unsigned comps, const bool flux, const CellK<T>& k, const PolyTab<T>& btab,
+                          const T* __restrict__ vtab, T* __restrict__ dst, const size_t row_pitch, const size_t obs_stride,
+                          const int nfx, const int jy0, const int n_rows, const EvalWalk& w, const int NT) {
+    if (flux) eval_rows_comps<T, true>(comps, k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else eval_rows_comps<T, false>(comps, k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
 }
 
 // a2 + a3 for one super-row of the fused kernel (S fine rows jy0 .. jy0+S-1 = one data row): thread `vt` takes the fine
@@ -740,7 +757,7 @@ __global__ void __launch_bounds__(256) k_fine(const __grid_constant__ FineParams
         }
         build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
         const CellK<T> k = load_cellk<T>(c);
-        eval_rows_any<T>(g.comps, k, p.btab, vtab, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy,
+        eval_rows_any<T>(g.comps, g.flux != 0, k, p.btab, vtab, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy,
                          make_walk(threadIdx.x, blockDim.x, g.nfx), blockDim.x);
     }
 }

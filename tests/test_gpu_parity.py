@@ -262,3 +262,49 @@ def test_jaffe_bulge_prior_batch(bang, oracle):
         ctx.close()
         assert_maps(maps, maps_o, prec, f"jaffe cfg2 {prec}")
         assert_logl(ll, logl_o, maps_o, data, err, mask, prec, near=near, what=f"jaffe cfg2 {prec}")
+
+
+# ------------------------------------------------------------------------------------------------ flux-weighted PSF (reading G')
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_flux_weighted_psf_config1_grid(bang, oracle, prec):
+    cfg = dict(W.config(1), psf_weighting=1)
+    theta = np.stack([W.theta_true(1), W.theta_true(1) * 1.01, W.theta_true(1) * 0.99])
+    theta[1, 0:2] = 0.37, -0.21
+    maps_o = oracle.model_maps(theta, cfg)
+    data, err, mask = W.make_data(1, maps_o[0])
+    logl_o, maps_o = oracle.loglike(theta, cfg, data, err, mask, return_maps=True)
+    ctx = bang.Context(cfg, precision=prec)
+    fine = ctx.model_fine(theta[:1]).cpu().numpy()[0]               # the four moment fields before the PSF
+    assert_maps(fine, oracle.model_fine(theta[0], cfg), prec, "flux fine")
+    ctx.set_data(data, err, mask)
+    maps = ctx.model_maps(theta).cpu().numpy()
+    ll = ctx.loglike(theta).cpu().numpy()
+    ctx.close()
+    assert_maps(maps, maps_o, prec, "flux maps")
+    assert_logl(ll, logl_o, maps_o, data, err, mask, prec, near=np.array([True, False, False]), what="flux cfg1")
+    plain = oracle.model_maps(theta[:1], W.config(1))[0]             # the paper's definition gives different kinematics
+    assert np.abs(maps_o[0, 1] / plain[1] - 1).max() > 0.05
+
+
+def test_flux_weighted_psf_prior_batch(bang, oracle):
+    # a seeded subset of config 2's prior-drawn batch, P = 2 launch shape; ragged 13 x 7 map with s = 3 in fp64
+    cfg = dict(W.config(2), psf_weighting=1)
+    theta = W.theta_batch(2)
+    sub = W.parity_subset(2, theta.shape[0], 24)
+    mtrue = oracle.model_maps(W.theta_true(2), cfg)[0]
+    data, err, mask = W.make_data(2, mtrue)
+    logl_o, maps_o = oracle.loglike(theta[sub], cfg, data, err, mask, return_maps=True)
+    near = np.isin(sub, W.near_truth_slots(2, theta.shape[0]))
+    for prec in ("fp32", "fp64"):
+        ctx = bang.Context(cfg, precision=prec)
+        ctx.set_data(data, err, mask)
+        maps = ctx.model_maps(theta[sub]).cpu().numpy()
+        ll = ctx.loglike(theta[sub]).cpu().numpy()
+        ctx.close()
+        assert_maps(maps, maps_o, prec, f"flux cfg2 {prec}")
+        assert_logl(ll, logl_o, maps_o, data, err, mask, prec, near=near, what=f"flux cfg2 {prec}")
+    small = dict(cfg, nx=13, ny=7)
+    ctx = bang.Context(small, precision="fp64")
+    got = ctx.model_maps(theta[sub][:4]).cpu().numpy()
+    ctx.close()
+    assert_maps(got, oracle.model_maps(theta[sub][:4], small), "fp64", "flux ragged")
