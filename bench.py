@@ -159,10 +159,12 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------ GPU legs
-def make_context(bang, idx, prec, variant=None):
-    """Context with synthetic data of the config: model(theta_true) from the library's own fp64 mode + seeded noise."""
+def make_context(bang, idx, prec, variant=None, extra=None):
+    """Context with synthetic data of the config: model(theta_true) from the library's own fp64 mode + seeded noise.
+    extra: overrides of the config (bulge_profile, psf_weighting: the widened variants of SURVEY.md sec. 8f)."""
     cfg = W.config(idx, variant)
-    c64 = bang.Context(W.config(idx), precision="fp64")
+    cfg.update(extra or {})
+    c64 = bang.Context(dict(W.config(idx), **(extra or {})), precision="fp64")
     mtrue = c64.model_maps(W.theta_true(idx)).cpu().numpy()[0]
     c64.close()
     data, err, mask = W.make_data(idx, mtrue)
@@ -278,10 +280,11 @@ def run_ours(args):
 
     if rank == 0 and world == 1 and not args.no_sweep:
         sweep = []
-        for (i2, p2, var) in [(2, "fp32", None), (2, "fp64", None), (3, "fp32", None), (3, "fp64", None),
-                              (4, "fp32", "B+D"), (4, "fp32", "B+2D"), (4, "fp32", "2D+H"), (4, "fp32", "B+2D+H"),
-                              (5, "fp32", None)]:
-            c2, cf2 = make_context(bang, i2, p2, var)
+        for (i2, p2, var, extra) in [(2, "fp32", None, None), (2, "fp64", None, None), (3, "fp32", None, None),
+                                     (3, "fp64", None, None), (4, "fp32", "B+D", None), (4, "fp32", "B+2D", None),
+                                     (4, "fp32", "2D+H", None), (4, "fp32", "B+2D+H", None), (5, "fp32", None, None),
+                                     (2, "fp32", "jaffe", {"bulge_profile": 1}), (2, "fp32", "fluxpsf", {"psf_weighting": 1})]:
+            c2, cf2 = make_context(bang, i2, p2, var if extra is None else None, extra)
             n2, rk2 = fine_cells(cf2)
             th2 = torch.as_tensor(W.theta_batch(i2), device="cuda")
             o2 = torch.empty(th2.shape[0], dtype=torch.float64, device="cuda")
@@ -290,6 +293,8 @@ def run_ours(args):
             sweep.append({"workload": workload_name(i2, p2) + (f"_{var}" if var else ""), "B": th2.shape[0],
                           "ms_per_step": 1e3 * statistics.mean(ts), "evals_per_s": th2.shape[0] / statistics.mean(ts),
                           "roofline_frac": r2["frac"], "clk_per_cell": r2["clk_per_cell_measured"]})
+            if extra and extra.get("psf_weighting"):
+                sweep[-1]["note"] = "side variant, run UNFUSED through HBM scratch (DESIGN.md sec. 11): not the tuned path"
             c2.close()
         line["sweep"] = sweep
     if rank == 0:
