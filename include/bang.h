@@ -96,7 +96,8 @@ typedef struct {
  * Jeans integral I~(s), the Freeman-disc function F(y)) once, on the device.  Synchronises the
  * stream before returning.  grid/psf/model are HOST pointers, copied.  On failure *out is NULL.
  * BANG_EINVAL: nx,ny < 1, s < 1 or s > 4, pix/dist <= 0, sigma < 0, no luminous component, unknown profile or
- * precision, a PSF whose footprint (2 r_k + s)/s exceeds 13 data pixels, or a row too wide for shared memory. */
+ * precision, a PSF whose footprint (2 r_k + s)/s exceeds 13 data pixels, or a row too wide for one CTA (nx > 512 in
+ * fp32 mode, nx > 256 in fp64 mode) or for shared memory. */
 int bang_create(bang_ctx **out, const bang_grid *grid, const bang_psf *psf, const bang_model *model,
                 int device, void *cuda_stream);
 

@@ -57,10 +57,16 @@ def synth_data(oracle, cfg, theta, seed=3):
     dict(nx=7, ny=9, supersample=4, sigma_pix=1.5, components=B_ | D1, halo_profile=W.HALO_HERNQUIST),
     dict(nx=8, ny=8, supersample=2, sigma_pix=1.0, components=D1 | D2 | H_, halo_profile=W.HALO_HERNQUIST),
     dict(nx=140, ny=3, supersample=2, sigma_pix=1.0),           # wide row: the P = 4 pixel-group path in fp32
+    dict(nx=300, ny=2, supersample=2, sigma_pix=1.0),           # wider still: the 512-thread launch class (fp64: 2 x 300 > 512 is refused)
 ])
 def test_shapes_and_variants_match_the_oracle(bang, oracle, kw, prec, tol):
     cfg = small_cfg(**kw)
     th = np.stack([THETA, THETA * np.array([1, 1, 2.5, 0.6, 1, 3, 1, 0.5, 1, 1, 1, 1, 1, 1, 1, -1, 1])])
+    if prec == "fp64" and cfg["nx"] > 256:                       # include/bang.h: fp64 mode holds rows of <= 256 pixels
+        with pytest.raises(bang.BangError) as e:
+            bang.Context(cfg, precision=prec)
+        assert e.value.code == bang.EINVAL
+        return
     ctx = bang.Context(cfg, precision=prec)
     maps = ctx.model_maps(th).cpu().numpy()
     fine = ctx.model_fine(th).cpu().numpy()
