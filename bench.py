@@ -2,12 +2,15 @@
 """bench.py -- likelihood evaluations per second of the batched BANG likelihood on B200 (driver contract).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4|5] [--precision fp32|fp64]
-                    [--impl ours|reference] [--no-sweep]
+                    [--impl ours|reference] [--scaling weak|strong] [--no-sweep] [--no-cpu]
 
 A "step" is one pass of the whole hot path (decode -> radial table -> fine cells -> PSF + rebin -> masked chi-square)
-over one batch of synthetic theta: one bang_loglike call.  Default workload: BASELINE.json configs[1] (B = 1024 theta,
-64 x 64 map, x3 supersampling, four-component model, fp32 compute with fp64 logL accumulation).  Prints ONE JSON line.
+over one batch of synthetic theta: one bang_loglike call.  Default workload: BASELINE.json configs[2], the live-point
+batch (B = 16384 theta, 128 x 128 map, 30 % mask, x3 supersampling, four-component model, fp32 compute with fp64 logL
+accumulation) -- the largest batch of the single-GPU configs; configs 2, 3 (fp64), 4 (four variants) and 5 follow as
+`sweep` rows, each with its own steps, clocks, end-to-end figure and roofline.  Prints ONE JSON line.
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload instead.
+`--scaling strong` (N > 1) shards ONE config batch over the ranks and all-gathers logL (dist.loglike_sharded).
 """
 from __future__ import annotations
 
@@ -123,6 +126,16 @@ class OracleLeg:
         assert np.isfinite(ll).all()
         return dt
 
+    def single_thread(self):
+        """one theta, one thread."""
+        n0 = self.bo.get_threads()
+        self.bo.set_threads(1)
+        try:
+            dt = self.run(np.arange(1))
+        finally:
+            self.bo.set_threads(n0)
+        return {"value": 1.0 / dt, "unit": UNIT, "cores": 1, "sample": f"1 theta, 1 thread, {dt:.2f} s wall"}
+
     def sample(self, budget_s, offset=0, max_n=4096):
         n = int(max(1, min(max_n, budget_s / max(self.t1, 1e-3))))
         B = self.theta.shape[0]
@@ -159,143 +172,206 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------ GPU legs
-def make_context(bang, idx, prec, variant=None, extra=None):
+COMP_NAMES = {1: "bulge", 2: "disc1", 4: "disc2", 8: "nfw"}
+
+
+def comp_string(comps):
+    return "+".join(n for b, n in COMP_NAMES.items() if comps & b)
+
+
+def make_context(bang, idx, prec, device, variant=None, extra=None):
     """Context with synthetic data of the config: model(theta_true) from the library's own fp64 mode + seeded noise.
     extra: overrides of the config (bulge_profile, psf_weighting: the widened variants of SURVEY.md sec. 8f)."""
     cfg = W.config(idx, variant)
     cfg.update(extra or {})
-    c64 = bang.Context(dict(W.config(idx), **(extra or {})), precision="fp64")
+    c64 = bang.Context(dict(W.config(idx), **(extra or {})), precision="fp64", device=device)
     mtrue = c64.model_maps(W.theta_true(idx)).cpu().numpy()[0]
     c64.close()
     data, err, mask = W.make_data(idx, mtrue)
-    ctx = bang.Context(cfg, precision=prec)
+    ctx = bang.Context(cfg, precision=prec, device=device)
     ctx.set_data(data, err, mask)
     return ctx, cfg
 
 
 def time_steps(torch, ctx, theta_dev, out, steps, warmup, flush):
-    for _ in range(warmup):
-        ctx.loglike(theta_dev, out)
-    torch.cuda.synchronize()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-    n0 = ctx.launches
-    for e0, e1 in ev:
-        flush.add_(1.0)                                        # L2 flush: rewrite a 256 MiB buffer (untimed)
-        e0.record()
-        ctx.loglike(theta_dev, out)
-        e1.record()
-    torch.cuda.synchronize()
+    """CUDA events on the context's stream (the stream the kernels are launched on) around each bang_loglike call."""
+    assert theta_dev.device == ctx.device == out.device == flush.device
+    stream = ctx.stream
+    with torch.cuda.stream(stream):
+        for _ in range(warmup):
+            ctx.loglike(theta_dev, out)
+        stream.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        n0 = ctx.launches
+        for e0, e1 in ev:
+            flush.add_(1.0)                                    # L2 flush: rewrite a 256 MiB buffer (untimed)
+            e0.record(stream)
+            ctx.loglike(theta_dev, out)
+            e1.record(stream)
+        stream.synchronize()
     return [e0.elapsed_time(e1) * 1e-3 for e0, e1 in ev], ctx.launches - n0
+
+
+def time_e2e(torch, ctx, theta_np, steps, warmup, flush):
+    """HOST theta -> bang_loglike_host -> HOST logL (pinned staging, H2D, kernels, D2H inside the call): host wall
+    clock per call; the L2 flush between calls is not timed."""
+    host_out = np.empty(theta_np.shape[0])
+    for _ in range(warmup):
+        ctx.loglike_host(theta_np, host_out)
+    total = 0.0
+    for _ in range(steps):
+        flush.add_(1.0)
+        torch.cuda.synchronize(ctx.device)
+        t0 = time.perf_counter()
+        ctx.loglike_host(theta_np, host_out)
+        total += time.perf_counter() - t0
+    assert np.isfinite(host_out).all()
+    return total
+
+
+def profile_numbers(name):
+    """DRAM bytes per k_fused launch and FMA-pipe utilisation from the committed ncu captures (profiles/traffic.csv)."""
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")
+    if os.path.exists(tp):
+        import csv
+        for row in csv.DictReader(open(tp)):
+            if row["workload"] == name:
+                fma = row.get("fma_pipe_pct")
+                return float(row["dram_bytes_per_launch"]), (float(fma) if fma not in (None, "") else None)
+    return None, None
+
+
+def measure(torch, bang, idx, prec, device, flush, steps, warmup, variant=None, extra=None, world=1, tag=None):
+    """One workload: device-timed steps (+ clocks), the end-to-end leg and the roofline object."""
+    ctx, cfg = make_context(bang, idx, prec, device, variant, extra)
+    ncell, rk = fine_cells(cfg)
+    theta_np = W.theta_batch(idx)
+    B = theta_np.shape[0]
+    theta_dev = torch.as_tensor(theta_np, device=ctx.device)
+    out = torch.empty(B, dtype=torch.float64, device=ctx.device)
+    e2e_t = D.max_over_ranks(time_e2e(torch, ctx, theta_np, steps, max(3, warmup), flush), device="cuda" if world > 1 else None)
+    if world > 1:
+        torch.distributed.barrier()
+    torch.cuda.synchronize(ctx.device)
+    with ClockSampler(index=device) as clk:
+        times, launches = time_steps(torch, ctx, theta_dev, out, steps, max(3, warmup), flush)
+    torch.cuda.synchronize(ctx.device)
+    if world > 1:
+        torch.distributed.barrier()
+    assert torch.isfinite(out).all()
+    total = D.max_over_ranks(sum(times), device="cuda" if world > 1 else None)
+    name = workload_name(idx, prec) + (f"_{tag or variant}" if (tag or variant) else "")
+    clocks = clk.summary()
+    unfused = bool(extra and extra.get("psf_weighting")) and not getattr(bang, "FLUX_IS_FUSED", False)
+    res = {"workload": name, "B": B, "steps": steps, "ms_per_step": 1e3 * total / steps,
+           "value": world * B * steps / total, "ncell": ncell, "rk": rk, "cfg": cfg, "launches": launches,
+           "e2e": {"value": world * B * steps / e2e_t, "unit": UNIT, "h2d_bytes_per_step": B * W.NTHETA * 8,
+                   "d2h_bytes_per_step": B * 8},
+           "clocks": clocks}
+    if not unfused:
+        traffic, fma = profile_numbers(name)
+        mean_t = total / steps
+        roof = R.roofline(B * ncell, mean_t, cfg["supersample"], rk, prec, clocks.get("sm_mhz"), traffic,
+                          comps=cfg["components"], fma_pipe_pct=fma)
+        roof["kernel"] = "k_fused"
+        roof["kernel_ms_best"] = 1e3 * min(times)
+        res["roofline"] = roof
+    res["ctx"] = ctx
+    return res
+
+
+SWEEP = [  # (config, precision, config-4 variant, overrides, tag)
+    (2, "fp32", None, None, None), (2, "fp64", None, None, None), (3, "fp64", None, None, None),
+    (4, "fp32", "B+D", None, None), (4, "fp32", "B+2D", None, None), (4, "fp32", "2D+H", None, None),
+    (4, "fp32", "B+2D+H", None, None), (5, "fp32", None, None, None),
+    (2, "fp32", None, {"bulge_profile": 1}, "jaffe"), (2, "fp32", None, {"psf_weighting": 1}, "fluxpsf"),
+    (2, "fp32", None, {"bulge_potential": 1}, "totalpot"),
+]
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` outside torchrun: start the N ranks ourselves (same contract as the driver's launch)."""
+    import subprocess
+    port = 29500 + os.getpid() % 2000
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
 
 def run_ours(args):
     import torch
     rank, world, local = D.env_rank_world()
-    if args.gpus > 1 or world > 1:
+    if args.gpus > 1 and world == 1:
+        if torch.cuda.device_count() < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but only {torch.cuda.device_count()} CUDA device(s) visible")
+        spawn_ranks(args)
+    if world > 1:
         import torch.distributed as dist
         torch.cuda.set_device(local)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    dev = torch.cuda.current_device()
+    dev = local if world > 1 else torch.cuda.current_device()
     from paper_2205_06819_b200 import bang                     # raises if libbang.so is missing: no fallback
 
     idx, prec = args.config, args.precision
-    ctx, cfg = make_context(bang, idx, prec)
-    ncell, rk = fine_cells(cfg)
-    theta_np = W.theta_batch(idx)                              # weak scaling: every rank runs the full config batch
-    B = theta_np.shape[0]
-    theta_dev = torch.as_tensor(theta_np, device="cuda")
-    out = torch.empty(B, dtype=torch.float64, device="cuda")
-    flush = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")
+    flush = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device=torch.device("cuda", dev))
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        cpu = OracleLeg(idx).sample(15.0)
-        cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        leg = OracleLeg(idx)
+        s = leg.sample(15.0)
+        cpu = {k: s[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        cpu["single_thread"] = leg.single_thread()
+        cpu["note"] = ("the oracle as it stands: direct evaluation per fine cell (N_J-node quadrature and 8 Bessel calls per "
+                       "cell, no tables), not an optimised CPU implementation")
 
-    # end-to-end leg: HOST theta -> bang_loglike_host -> HOST logL (pinned staging, H2D, kernel, D2H inside the call)
-    host_out = np.empty(B)
-    for _ in range(max(3, args.warmup)):
-        ctx.loglike_host(theta_np, host_out)
-    if world > 1:
-        torch.distributed.barrier()
-    torch.cuda.synchronize()
-    e2e_local = 0.0
-    for _ in range(args.steps):
-        flush.add_(1.0)                                        # L2 flush between steps, outside the timed call
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        ctx.loglike_host(theta_np, host_out)                   # returns after the D2H copy: host wall clock is the cost
-        e2e_local += time.perf_counter() - t0
-    e2e_t = D.max_over_ranks(e2e_local, device="cuda" if world > 1 else None)
-
-    # device-timed leg
-    if world > 1:
-        torch.distributed.barrier()
-    torch.cuda.synchronize()
-    with ClockSampler(index=dev) as clk:
-        times, launches = time_steps(torch, ctx, theta_dev, out, args.steps, max(3, args.warmup), flush)
-    torch.cuda.synchronize()
-    if world > 1:
-        torch.distributed.barrier()
-    total = D.max_over_ranks(sum(times), device="cuda" if world > 1 else None)
-    ms_step = 1e3 * total / args.steps
-    value = world * B * args.steps / total
-    clocks = clk.summary()
-    assert torch.isfinite(out).all()
-
-    traffic = None                                             # DRAM bytes per k_fused launch from the ncu capture
-    tp = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(tp):
-        import csv
-        for row in csv.DictReader(open(tp)):
-            if row["workload"] == workload_name(idx, prec):
-                traffic = float(row["dram_bytes_per_launch"])
-    roof = R.roofline(B * ncell, statistics.mean(times), cfg["supersample"], rk, prec, clocks.get("sm_mhz"), traffic)
-    roof["kernel"] = "k_fused"
-    roof["kernel_ms_best"] = 1e3 * min(times)
-    # measured counterparts of the derived peaks (dependency-free FFMA / MUFU / DFMA chains, bang_probe_peaks)
-    pk = ctx.probe_peaks()
-    cen = R.census(cfg["supersample"], rk, prec)
-    t_meas = B * ncell * (cen["fp64"] / pk["fp64_fma"] if prec == "fp64"
-                          else max(cen["fp32"] / pk["fp32_fma"], cen["mufu"] / pk["mufu"]))
-    roof["peaks_measured_Tinstr"] = {k: v / 1e12 for k, v in pk.items()}
-    roof["frac_of_measured_peaks"] = t_meas / statistics.mean(times)
-
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32" if prec == "fp32" else "f64", "data": "synthetic",
-            "config": {"workload": workload_name(idx, prec), "B_per_gpu": B, "nx": cfg["nx"], "ny": cfg["ny"],
-                       "supersample": cfg["supersample"], "sigma_pix": cfg["sigma_pix"], "r_k": rk,
-                       "jeans_nodes": cfg["jeans_nodes"], "fine_cells_per_theta": ncell,
-                       "components": "bulge+disc1+disc2+nfw", "logL_accumulation": "f64",
-                       "l2": "flushed between timed iterations (256 MiB rewrite)",
-                       "parallelism": f"theta-sharded x{world}, no data-path collective"},
-            "fine_cell_evals_per_s": value * ncell,
-            "e2e": {"value": world * B * args.steps / e2e_t, "unit": UNIT, "h2d_bytes_per_step": B * W.NTHETA * 8,
-                    "d2h_bytes_per_step": B * 8},
-            "gpu_launches": launches, "clocks": clocks, "roofline": roof}
+    if args.scaling == "strong" and world > 1:
+        line = run_strong(torch, bang, args, idx, prec, dev, flush, rank, world)
+    else:
+        m = measure(torch, bang, idx, prec, dev, flush, args.steps, args.warmup, world=world,
+                    variant="B+2D+H" if idx == 4 else None)
+        cfg, ctx = m["cfg"], m["ctx"]
+        roof = m["roofline"]
+        # measured counterparts of the derived peaks (dependency-free FFMA / MUFU / DFMA chains, bang_probe_peaks)
+        pk = ctx.probe_peaks()
+        cen = R.census(cfg["supersample"], m["rk"], prec, cfg["components"])
+        t_meas = m["B"] * m["ncell"] * (cen["fp64"] / pk["fp64_fma"] if prec == "fp64"
+                                        else max(cen["fp32"] / pk["fp32_fma"], cen["mufu"] / pk["mufu"]))
+        roof["peaks_measured_Tinstr"] = {k: v / 1e12 for k, v in pk.items()}
+        roof["frac_of_measured_peaks"] = t_meas / (1e-3 * m["ms_per_step"])
+        ctx.close()
+        line = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(3, args.warmup), "ms_per_step": m["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32" if prec == "fp32" else "f64", "data": "synthetic",
+                "config": {"workload": m["workload"], "B_per_gpu": m["B"], "nx": cfg["nx"], "ny": cfg["ny"],
+                           "supersample": cfg["supersample"], "sigma_pix": cfg["sigma_pix"], "r_k": m["rk"],
+                           "jeans_nodes": cfg["jeans_nodes"], "fine_cells_per_theta": m["ncell"],
+                           "components": comp_string(cfg["components"]), "logL_accumulation": "f64",
+                           "mask_frac": cfg.get("mask_frac", 0.0),
+                           "l2": "flushed between timed iterations (256 MiB rewrite)",
+                           "parallelism": f"theta-sharded x{world}, every rank runs the config batch, no data-path collective"},
+                "fine_cell_evals_per_s": m["value"] * m["ncell"], "e2e": m["e2e"], "gpu_launches": m["launches"],
+                "clocks": m["clocks"], "roofline": roof}
     if cpu is not None:
         line["cpu_baseline"] = cpu
-    ctx.close()
 
     if rank == 0 and world == 1 and not args.no_sweep:
         sweep = []
-        for (i2, p2, var, extra) in [(2, "fp32", None, None), (2, "fp64", None, None), (3, "fp32", None, None),
-                                     (3, "fp64", None, None), (4, "fp32", "B+D", None), (4, "fp32", "B+2D", None),
-                                     (4, "fp32", "2D+H", None), (4, "fp32", "B+2D+H", None), (5, "fp32", None, None),
-                                     (2, "fp32", "jaffe", {"bulge_profile": 1}), (2, "fp32", "fluxpsf", {"psf_weighting": 1})]:
-            c2, cf2 = make_context(bang, i2, p2, var if extra is None else None, extra)
-            n2, rk2 = fine_cells(cf2)
-            th2 = torch.as_tensor(W.theta_batch(i2), device="cuda")
-            o2 = torch.empty(th2.shape[0], dtype=torch.float64, device="cuda")
-            ts, _ = time_steps(torch, c2, th2, o2, 5, 3, flush)
-            r2 = R.roofline(th2.shape[0] * n2, statistics.mean(ts), cf2["supersample"], rk2, p2)
-            sweep.append({"workload": workload_name(i2, p2) + (f"_{var}" if var else ""), "B": th2.shape[0],
-                          "ms_per_step": 1e3 * statistics.mean(ts), "evals_per_s": th2.shape[0] / statistics.mean(ts),
-                          "roofline_frac": r2["frac"], "clk_per_cell": r2["clk_per_cell_measured"]})
-            if extra and extra.get("psf_weighting"):
-                sweep[-1]["note"] = "side variant, run UNFUSED through HBM scratch (DESIGN.md sec. 11): not the tuned path"
-            c2.close()
+        for (i2, p2, var, extra, tag) in SWEEP:
+            if (i2, p2) == (idx, prec) and var is None and extra is None:
+                continue
+            if extra and "bulge_potential" in extra and not getattr(bang, "HAS_TOTAL_POTENTIAL", False):
+                continue
+            r = measure(torch, bang, i2, p2, dev, flush, max(20, min(args.steps, 50)), 3, var, extra, tag=tag)
+            r.pop("ctx").close()
+            r.pop("cfg")
+            row = {"workload": r["workload"], "B": r["B"], "steps": r["steps"], "ms_per_step": r["ms_per_step"],
+                   "evals_per_s": r["value"], "e2e": r["e2e"], "clocks": r["clocks"], "gpu_launches": r["launches"]}
+            if "roofline" in r:
+                row["roofline"] = r["roofline"]
+                row["roofline_frac"] = r["roofline"]["frac"]
+            else:
+                row["note"] = "side variant run UNFUSED through HBM scratch: no roofline is claimed for it"
+            sweep.append(row)
         line["sweep"] = sweep
     if rank == 0:
         print(json.dumps(line))
@@ -303,14 +379,55 @@ def run_ours(args):
         torch.distributed.destroy_process_group()
 
 
+def run_strong(torch, bang, args, idx, prec, dev, flush, rank, world):
+    """SURVEY.md sec. 8(e) as one call: shard theta[B] over the ranks, evaluate, all-gather logL (strong scaling)."""
+    ctx, cfg = make_context(bang, idx, prec, dev, "B+2D+H" if idx == 4 else None)
+    ncell, rk = fine_cells(cfg)
+    theta_np = W.theta_batch(idx)
+    B = theta_np.shape[0]
+    theta_dev = torch.as_tensor(theta_np, device=ctx.device)
+    for _ in range(max(3, args.warmup)):
+        full = D.loglike_sharded(ctx, theta_dev)
+    torch.cuda.synchronize(ctx.device)
+    torch.distributed.barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    with ClockSampler(index=dev) as clk:
+        for e0, e1 in ev:
+            flush.add_(1.0)
+            e0.record()
+            full = D.loglike_sharded(ctx, theta_dev)
+            e1.record()
+        torch.cuda.synchronize(ctx.device)
+    torch.distributed.barrier()
+    assert full.shape == (B,) and torch.isfinite(full).all()
+    total = D.max_over_ranks(sum(e0.elapsed_time(e1) * 1e-3 for e0, e1 in ev), device="cuda")
+    lo, hi = D.shard_bounds(B, rank, world)
+    roof = R.roofline(B * ncell / world, total / args.steps, cfg["supersample"], rk, prec, clk.summary().get("sm_mhz"),
+                      None, comps=cfg["components"])
+    roof["kernel"] = "k_fused"
+    ctx.close()
+    return {"metric": METRIC, "value": B * args.steps / total, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f32" if prec == "fp32" else "f64", "data": "synthetic",
+            "config": {"workload": workload_name(idx, prec), "B_total": B, "B_per_gpu": hi - lo, "nx": cfg["nx"], "ny": cfg["ny"],
+                       "supersample": cfg["supersample"], "fine_cells_per_theta": ncell,
+                       "l2": "flushed between timed iterations (256 MiB rewrite)",
+                       "parallelism": f"ONE batch sharded x{world} (dist.loglike_sharded), all-gather of logL inside the timed region"},
+            "fine_cell_evals_per_s": B * args.steps / total * ncell,
+            "e2e": {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                    "note": "not measured in the strong-scaling mode"},
+            "gpu_launches": 2 * args.steps, "clocks": clk.summary(), "roofline": roof}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=3, choices=[2, 3, 4, 5])
     ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

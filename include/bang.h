@@ -97,7 +97,10 @@ typedef struct {
  * stream before returning.  grid/psf/model are HOST pointers, copied.  On failure *out is NULL.
  * BANG_EINVAL: nx,ny < 1, s < 1 or s > 4, pix/dist <= 0, sigma < 0, no luminous component, unknown profile or
  * precision, a PSF whose footprint (2 r_k + s)/s exceeds 13 data pixels, or a row too wide for one CTA (nx > 512 in
- * fp32 mode, nx > 256 in fp64 mode) or for shared memory. */
+ * fp32 mode, nx > 256 in fp64 mode) or for shared memory.
+ * The calling thread's current CUDA device is left as it was found, here and in every other call.
+ * The launch shape is derived from the grid alone; a development build (-DBANG_TUNING) can override it from the
+ * environment (BANG_P, BANG_THREADS, BANG_CTAS, BANG_VERBOSE) -- the default build reads no environment variable. */
 int bang_create(bang_ctx **out, const bang_grid *grid, const bang_psf *psf, const bang_model *model,
                 int device, void *cuda_stream);
 
@@ -111,8 +114,14 @@ int bang_set_data(bang_ctx *ctx, const double *data_dev, const double *err_dev, 
 
 /* Model maps for a batch: theta_dev DEVICE [B][17] doubles; maps_dev DEVICE [B][4][ny][nx], float if the context is
  * BANG_FP32, double if BANG_FP64 (map order as above; B in linear units).  theta outside the model's domain (R <= 0,
- * M/L <= 0, |k| > 1, |i| >= 90 deg, non-finite entries of a present component, or radii outside the tabulated range
- * 2^-22 <= R/R_b <= 2^18, r < 2^26 kpc) is not an error: its maps are NaN.  B = 0 is a no-op.  Asynchronous. */
+ * M/L <= 0, |k| > 1, |i| >= 90 deg, non-finite entries of a present component) is not an error: its maps are NaN.
+ * The library's domain is the model's, not its tables': a theta whose radii leave the tabulated ranges of the fused
+ * kernel (more than 32 octaves of r^2 on the grid, R/R_b outside [2^-22, 2^18), or i > 89.1 deg in BANG_FP32 mode, where
+ * fp32 coordinates no longer carry r) is evaluated by a second, direct kernel (eq. 4-5 in closed form, eq. 6 by the
+ * N_J-node rule, eq. 10 term by term, fp64 geometry; ~1e3 times slower per theta), launched after the fused one in every
+ * call and empty for any theta of a sensible prior box.  Only on a grid whose row does not fit that kernel's shared
+ * memory (4 (nx s + 2 r_k) + 4 NACC nx values) are such theta reported as out of domain.  B = 0 is a no-op.
+ * Asynchronous. */
 int bang_model_maps(bang_ctx *ctx, const double *theta_dev, int B, void *maps_dev);
 
 /* Un-convolved model on the supersampled grid, the intermediate of the path before the PSF (App. A Alg. 1 line 3,

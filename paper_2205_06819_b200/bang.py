@@ -80,7 +80,13 @@ def lib():
 
 
 class Context:
-    """One bang_ctx: a grid, a PSF, a model variant and a precision, bound to a CUDA device and stream."""
+    """One bang_ctx: a grid, a PSF, a model variant and a precision, bound to a CUDA device and stream.
+
+    Every kernel is enqueued on the context's stream (`ctx.stream`: the stream given at construction, else the device's
+    current stream at that moment).  The temporaries this binding makes (theta uploaded from the host, output tensors)
+    are allocated and filled under that same stream, so a caller working on another stream only has to order its own
+    tensors against `ctx.stream` (torch.cuda.Stream.wait_stream).  The C entry points leave the calling thread's
+    current CUDA device as they found it."""
 
     def __init__(self, cfg: dict, precision: str | None = None, device: int = 0, stream=None):
         import torch
@@ -114,6 +120,13 @@ class Context:
         if rc != OK:
             raise BangError(rc, lib().bang_last_error(self._h).decode() or lib().bang_strerror(rc).decode())
 
+    @property
+    def stream(self):
+        return self._stream
+
+    def _on_stream(self):
+        return self._torch.cuda.stream(self._stream)
+
     def _theta(self, theta):
         torch = self._torch
         t = torch.as_tensor(theta, dtype=torch.float64, device=self.device).reshape(-1, NTHETA).contiguous()
@@ -142,34 +155,38 @@ class Context:
         m = torch.as_tensor(np.asarray(mask, dtype=np.uint8) if not torch.is_tensor(mask) else mask,
                             dtype=torch.uint8, device=self.device).contiguous()
         assert d.shape == (4, self.ny, self.nx) and e.shape == d.shape and m.shape == d.shape
+        torch.cuda.current_stream(self.device).synchronize()         # the uploads above ran on the current stream
         self._check(lib().bang_set_data(self._h, d.data_ptr(), e.data_ptr(), m.data_ptr()))
 
     def model_maps(self, theta, out=None):
         """theta [B][17] (tensor on the device, or array-like) -> maps [B][4][ny][nx] device tensor (async)."""
         torch = self._torch
-        t = self._theta(theta)
-        B = t.shape[0]
-        if out is None:
-            out = torch.empty((B, 4, self.ny, self.nx), dtype=self.dtype, device=self.device)
-        self._check(lib().bang_model_maps(self._h, t.data_ptr(), B, out.data_ptr()))
+        with self._on_stream():
+            t = self._theta(theta)
+            B = t.shape[0]
+            if out is None:
+                out = torch.empty((B, 4, self.ny, self.nx), dtype=self.dtype, device=self.device)
+            self._check(lib().bang_model_maps(self._h, t.data_ptr(), B, out.data_ptr()))
         return out
 
     def model_fine(self, theta):
         torch = self._torch
-        t = self._theta(theta)
-        B = t.shape[0]
-        out = torch.empty((B, 4, self.nfy, self.nfx), dtype=self.dtype, device=self.device)
-        self._check(lib().bang_model_fine(self._h, t.data_ptr(), B, out.data_ptr()))
+        with self._on_stream():
+            t = self._theta(theta)
+            B = t.shape[0]
+            out = torch.empty((B, 4, self.nfy, self.nfx), dtype=self.dtype, device=self.device)
+            self._check(lib().bang_model_fine(self._h, t.data_ptr(), B, out.data_ptr()))
         return out
 
     def loglike(self, theta, out=None):
         """theta [B][17] device tensor -> logL [B] float64 device tensor (async on the context's stream)."""
         torch = self._torch
-        t = self._theta(theta)
-        B = t.shape[0]
-        if out is None:
-            out = torch.empty((B,), dtype=torch.float64, device=self.device)
-        self._check(lib().bang_loglike(self._h, t.data_ptr(), B, out.data_ptr()))
+        with self._on_stream():
+            t = self._theta(theta)
+            B = t.shape[0]
+            if out is None:
+                out = torch.empty((B,), dtype=torch.float64, device=self.device)
+            self._check(lib().bang_loglike(self._h, t.data_ptr(), B, out.data_ptr()))
         return out
 
     def loglike_host(self, theta: np.ndarray, out: np.ndarray | None = None) -> np.ndarray:

@@ -10,6 +10,7 @@
 #include "../../include/bang.h"
 #include "bang_host.h"
 #include "bang_moments.cuh"
+#include "bang_slow.cuh"
 
 using namespace bang;
 
@@ -28,12 +29,16 @@ struct bang_ctx {
     void* Ftab = nullptr; int Ftab_first = 0, Ftab_cells = 0;
     double2* data = nullptr; double C0 = 0.0; bool has_data = false;
     double* scal = nullptr;                // device scratch: {C0, bad-pixel count}
+    double* gl_dev = nullptr;              // N_J Gauss-Legendre nodes then weights (reading B): table build, direct path
     // staging for the *_host calls
     double* h_theta = nullptr; double* d_theta = nullptr; void* h_out = nullptr; void* d_out = nullptr;
     size_t cap_theta = 0, cap_out = 0;
     long long launches = 0;
     int force_ctas = 0;
     int launch_cache[2] = {0, 0};
+    // direct path (bang_slow.cuh): list of the theta k_fused leaves to k_slow, {count, CTAs done}, capacity; 0 = the grid
+    // is too large for k_slow's shared memory (such theta are then reported as out of domain)
+    int* slow_list = nullptr; int* slow_cnt = nullptr; int slow_cap = 0; size_t slow_smem = 0;
     // flux-weighted PSF variant (unfused): composite taps on the device, scratch for the moment fields of a chunk of theta
     double* W_dev = nullptr; void* fx_fine = nullptr; int* fx_valid = nullptr; double* fx_chi2 = nullptr;
     int fx_chunk = 0; size_t fx_chi2_cap = 0;          // per mode: resident CTAs per SM once the kernel is configured
@@ -58,6 +63,23 @@ int fail(bang_ctx* c, int code, const char* fmt, ...) {
             return fail(ctx, e_ == cudaErrorMemoryAllocation ? BANG_ENOMEM : BANG_ECUDA, "%s: %s", #call,    \
                         cudaGetErrorString(e_));                                                              \
     } while (0)
+
+// Every entry point runs on the context's device and leaves the calling thread's current device as it found it.
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        ok = (prev == dev) || cudaSetDevice(dev) == cudaSuccess;
+        if (prev == dev) prev = -1;                    // nothing to restore
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+#define ON_DEVICE(ctx)                                                                       \
+    DeviceGuard dev_guard_((ctx)->device);                                                   \
+    if (!dev_guard_.ok) return fail((ctx), BANG_ECUDA, "cudaSetDevice(%d) failed", (ctx)->device)
 
 // Gauss-Legendre nodes and weights on (-1,1): Newton iteration on P_n (Abramowitz & Stegun 25.4.29), long double
 void gauss_legendre(int n, double* x, double* w) {
@@ -231,6 +253,7 @@ int build_universal(bang_ctx* ctx, const double* glx_dev, const double* glw_dev)
     double* vals = nullptr;
     const size_t nb = (size_t)ctx->btab_cells * 2 * NC, nf = (size_t)ctx->Ftab_cells * NC;
     CU(cudaMalloc(&vals, (nb + nf) * sizeof(double)));
+    struct Free { double* p; ~Free() { cudaFree(p); } } free_vals{vals};      // also on the error returns below
     CU(cudaMalloc(&ctx->btab, nb * sizeof(T)));
     CU(cudaMalloc(&ctx->Ftab, nf * sizeof(T)));
     const int th = 128;
@@ -245,7 +268,6 @@ int build_universal(bang_ctx* ctx, const double* glx_dev, const double* glw_dev)
     ctx->launches += 4;
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(ctx->stream));
-    cudaFree(vals);
     return BANG_OK;
 }
 
@@ -270,7 +292,54 @@ FusedLaunch make_launch(bang_ctx* c, const double* theta, int B, int mode, void*
     L.maps = maps; L.data = c->data; L.C0 = c->C0; L.logL = logL;
     L.threads = c->threads; L.ctas = c->force_ctas; L.n_sm = c->n_sm; L.stream = c->stream;
     L.cache = c->launch_cache;
+    L.slow_list = c->slow_smem ? c->slow_list : nullptr; L.slow_count = c->slow_cnt;
     return L;
+}
+
+// pitch of the data array's pixel-group axis: the launch-bound class of the fused kernel / 4 (lbc_threads)
+int data_gmax(const bang_ctx* c) { return (c->threads <= 128 ? 128 : (c->threads <= 256 ? 256 : 512)) / 4; }
+
+// room for B entries in the list of theta that take the direct path
+int ensure_slow_list(bang_ctx* ctx, int B) {
+    if (!ctx->slow_smem || B <= ctx->slow_cap) return BANG_OK;
+    CU(cudaStreamSynchronize(ctx->stream));
+    cudaFree(ctx->slow_list); ctx->slow_list = nullptr; ctx->slow_cap = 0;
+    CU(cudaMalloc(&ctx->slow_list, (size_t)B * sizeof(int)));
+    ctx->slow_cap = B;
+    return BANG_OK;
+}
+
+// the direct path for the theta k_fused recorded (an empty list costs one empty launch)
+template <typename T>
+int run_slow(bang_ctx* ctx, const double* theta_dev, int mode, void* maps_dev, double* logL_dev) {
+    if (!ctx->slow_smem) return BANG_OK;
+    SlowParams<T> p{};
+    p.g = ctx->g;
+    p.btab = PolyTab<T>{static_cast<const T*>(ctx->btab), ctx->btab_first, ctx->btab_cells};
+    p.Ftab = PolyTab<T>{static_cast<const T*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells};
+    p.direct = DirectC{ctx->gl_dev, ctx->gl_dev + ctx->model.jeans_nodes, ctx->model.jeans_nodes};
+    p.W = ctx->W_dev; p.nacc = ctx->nacc;
+    p.theta = theta_dev; p.slow_list = ctx->slow_list; p.slow_count = ctx->slow_cnt; p.done = ctx->slow_cnt + 1;
+    p.maps = static_cast<T*>(maps_dev); p.data = ctx->data; p.P = ctx->P; p.gmax = data_gmax(ctx);
+    p.C0 = ctx->C0; p.logL = logL_dev;
+    if (mode == 0) k_slow<T, 0><<<ctx->n_sm, 256, ctx->slow_smem, ctx->stream>>>(p);
+    else k_slow<T, 1><<<ctx->n_sm, 256, ctx->slow_smem, ctx->stream>>>(p);
+    ctx->launches += 1;
+    CU(cudaGetLastError());
+    return BANG_OK;
+}
+template <typename T>
+int setup_slow(bang_ctx* ctx) {
+    const size_t smem = slow_smem_bytes<T>(ctx->g, ctx->nacc);
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, ctx->device));
+    if (smem > prop.sharedMemPerBlockOptin) return BANG_OK;          // slow_smem stays 0: no direct path on this grid
+    CU(cudaFuncSetAttribute(k_slow<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU(cudaFuncSetAttribute(k_slow<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU(cudaMalloc(&ctx->slow_cnt, 2 * sizeof(int)));
+    CU(cudaMemsetAsync(ctx->slow_cnt, 0, 2 * sizeof(int), ctx->stream));
+    ctx->slow_smem = smem;
+    return BANG_OK;
 }
 
 int ensure_staging(bang_ctx* ctx, int B, size_t out_bytes) {
@@ -300,11 +369,6 @@ int run_flux(bang_ctx* ctx, const double* theta_dev, int B, int mode, void* maps
     const GridC& g = ctx->g;
     const size_t plane4 = (size_t)4 * g.nfx * g.nfy * sizeof(T);
     const int ntap = 2 * ctx->rk + g.s;
-    if (!ctx->W_dev) {
-        CU(cudaMalloc(&ctx->W_dev, ntap * sizeof(double)));
-        CU(cudaMemcpyAsync(ctx->W_dev, ctx->W.data(), ntap * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-        CU(cudaStreamSynchronize(ctx->stream));                      // ctx->W is pageable host memory
-    }
     if (!ctx->fx_fine) {                                              // scratch: at most 256 MiB of moment fields
         ctx->fx_chunk = (int)std::max<size_t>(1, std::min<size_t>(4096, ((size_t)256 << 20) / plane4));
         CU(cudaMalloc(&ctx->fx_fine, (size_t)ctx->fx_chunk * plane4));
@@ -317,14 +381,15 @@ int run_flux(bang_ctx* ctx, const double* theta_dev, int B, int mode, void* maps
     }
     const size_t smem = fused_smem_bytes<T>(0, 0);
     CU(cudaFuncSetAttribute(k_fine<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int gmax = (ctx->threads <= 128 ? 128 : (ctx->threads <= 256 ? 256 : 512)) / 4;
+    const int gmax = data_gmax(ctx);
+    const DirectC direct{ctx->gl_dev, ctx->gl_dev + ctx->model.jeans_nodes, ctx->model.jeans_nodes};
     for (int b0 = 0; b0 < B; b0 += ctx->fx_chunk) {
         const int Bc = std::min(ctx->fx_chunk, B - b0);
         const double* th = theta_dev + (size_t)b0 * kNTheta;
-        k_theta_valid<T><<<(Bc + 127) / 128, 128, 0, ctx->stream>>>(th, Bc, g, ctx->fx_valid);
+        const PolyTab<T> Ft{static_cast<const T*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells};
+        k_theta_valid<T><<<(Bc + 127) / 128, 128, 0, ctx->stream>>>(th, Bc, g, Ft, ctx->fx_valid);
         FineParams<T> fp{g, ctx->fit, PolyTab<T>{static_cast<const T*>(ctx->btab), ctx->btab_first, ctx->btab_cells},
-                         PolyTab<T>{static_cast<const T*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells}, th, Bc,
-                         static_cast<T*>(ctx->fx_fine)};
+                         Ft, direct, th, Bc, static_cast<T*>(ctx->fx_fine)};
         k_fine<T><<<std::min(Bc, 8 * ctx->n_sm), 256, smem, ctx->stream>>>(fp);
         MomentsParams<T> mp{g, ntap, ctx->W_dev, static_cast<const T*>(ctx->fx_fine), Bc, b0, ctx->fx_valid,
                             static_cast<T*>(maps_dev), ctx->data, ctx->P, gmax, ctx->fx_chi2, mode};
@@ -371,7 +436,8 @@ int bang_ml_from_colour(const double* m_beta_dev, const double* m_gamma_dev, con
                         double* ml_err_dev, int device, void* cuda_stream) {
     if (n < 0 || (n > 0 && (!m_beta_dev || !m_gamma_dev || !dm_beta_dev || !dm_gamma_dev || !ml_dev || !ml_err_dev))) return BANG_EINVAL;
     if (n == 0) return BANG_OK;
-    if (cudaSetDevice(device) != cudaSuccess) return BANG_ECUDA;
+    DeviceGuard dg(device);
+    if (!dg.ok) return BANG_ECUDA;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return BANG_ECUDA;
     const int threads = 256;
@@ -385,7 +451,7 @@ int bang_ml_from_colour(const double* m_beta_dev, const double* m_gamma_dev, con
 int bang_probe_peaks(bang_ctx* ctx, double* out_host) {
     if (!ctx) return BANG_EINVAL;
     if (!out_host) return fail(ctx, BANG_EINVAL, "bang_probe_peaks: null pointer");
-    CU(cudaSetDevice(ctx->device));
+    ON_DEVICE(ctx);
     float* sink = nullptr;
     CU(cudaMalloc(&sink, sizeof(float)));
     cudaEvent_t e0, e1;
@@ -416,10 +482,11 @@ int bang_probe_peaks(bang_ctx* ctx, double* out_host) {
 
 void bang_destroy(bang_ctx* ctx) {
     if (!ctx) return;
-    cudaSetDevice(ctx->device);
+    DeviceGuard dg(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    cudaFree(ctx->btab); cudaFree(ctx->Ftab); cudaFree(ctx->data); cudaFree(ctx->scal);
+    cudaFree(ctx->btab); cudaFree(ctx->Ftab); cudaFree(ctx->data); cudaFree(ctx->scal); cudaFree(ctx->gl_dev);
     cudaFree(ctx->d_theta); cudaFree(ctx->d_out);
+    cudaFree(ctx->slow_list); cudaFree(ctx->slow_cnt);
     cudaFree(ctx->W_dev); cudaFree(ctx->fx_fine); cudaFree(ctx->fx_valid); cudaFree(ctx->fx_chi2);
     if (ctx->h_theta) cudaFreeHost(ctx->h_theta);
     if (ctx->h_out) cudaFreeHost(ctx->h_out);
@@ -442,7 +509,6 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     if (model->jeans_nodes < 1 || model->jeans_nodes > 4096) return BANG_EINVAL;
     if (model->precision != BANG_FP32 && model->precision != BANG_FP64) return BANG_EINVAL;
     if (model->psf_weighting != BANG_PSF_FIELDS && model->psf_weighting != BANG_PSF_FLUX) return BANG_EINVAL;
-    if (model->psf_weighting != BANG_PSF_FIELDS && model->psf_weighting != BANG_PSF_FLUX) return BANG_EINVAL;
 
     const int s = grid->supersample;
     const int rk = (int)std::ceil(psf->trunc_nsigma * psf->sigma_pix * s - 1e-9);
@@ -451,7 +517,8 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return BANG_ECUDA;
-    if (cudaSetDevice(device) != cudaSuccess) return BANG_ECUDA;
+    DeviceGuard dg(device);
+    if (!dg.ok) return BANG_ECUDA;
 
     bang_ctx* ctx = new (std::nothrow) bang_ctx;
     if (!ctx) return BANG_ENOMEM;
@@ -470,7 +537,6 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     g.spx = s / grid->pix_arcsec;
     g.h = grid->pix_arcsec * grid->dist_mpc * kKpcPerArcsecPerMpc / s;
     g.comps = model->components; g.halo_profile = model->halo_profile; g.bulge_profile = model->bulge_profile;
-    g.flux = model->psf_weighting;
     g.flux = model->psf_weighting;
 
     // eq. 21 on the fine grid, separable (reading F): g[m] = exp(-m^2/(2 sigma_f^2)), normalised;
@@ -495,41 +561,45 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     }
 
     // launch shape: P data pixels per thread in the PSF phase, one thread per (observable, pixel group)
-    const char* envP = getenv("BANG_P");
     int P = f64 ? 2 : (grid->nx > 64 ? 4 : 2);        // measured: P = 4 wins from 80 columns on even with idle PSF threads
-    if (envP && !f64 && (atoi(envP) == 2 || atoi(envP) == 4)) P = atoi(envP);
+#ifdef BANG_TUNING      // development builds only (-DBANG_TUNING): sweep the launch shape from the environment
+    if (const char* e = getenv("BANG_P")) if (!f64 && (atoi(e) == 2 || atoi(e) == 4)) P = atoi(e);
+#endif
     ctx->P = P;
     ctx->nxp = (grid->nx + P - 1) / P * P;
     const int items = 4 * ctx->nxp / P;
     ctx->threads = std::max(128, (items + 31) / 32 * 32);
-    const char* envT = getenv("BANG_THREADS");
-    if (envT && atoi(envT) >= ctx->threads && atoi(envT) <= 512) ctx->threads = atoi(envT) / 32 * 32;
-    const char* envC = getenv("BANG_CTAS");
-    if (envC && atoi(envC) > 0) ctx->force_ctas = atoi(envC);
+#ifdef BANG_TUNING
+    if (const char* e = getenv("BANG_THREADS")) if (atoi(e) >= ctx->threads && atoi(e) <= 512) ctx->threads = atoi(e) / 32 * 32;
+    if (const char* e = getenv("BANG_CTAS")) if (atoi(e) > 0) ctx->force_ctas = atoi(e);
+#endif
     if (ctx->threads > 512) { delete ctx; return BANG_EINVAL; }      // row too wide for one CTA
     make_fit(f64 ? TabCfg<double>::D : TabCfg<float>::D, ctx->fit);
 
     // N_J-node Gauss-Legendre rule (reading B), then the scale-free tables on the device
     std::vector<double> gl(2 * (size_t)model->jeans_nodes);
     gauss_legendre(model->jeans_nodes, gl.data(), gl.data() + model->jeans_nodes);
-    double* gl_dev = nullptr;
     int rc = BANG_OK;
     do {
-        if (cudaMalloc(&gl_dev, gl.size() * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
-        if (cudaMemcpyAsync(gl_dev, gl.data(), gl.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess) {
+        if (cudaMalloc(&ctx->gl_dev, gl.size() * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
+        if (cudaMemcpyAsync(ctx->gl_dev, gl.data(), gl.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess) {
             rc = BANG_ECUDA; break;
         }
-        rc = f64 ? build_universal<double>(ctx, gl_dev, gl_dev + model->jeans_nodes)
-                 : build_universal<float>(ctx, gl_dev, gl_dev + model->jeans_nodes);
+        rc = f64 ? build_universal<double>(ctx, ctx->gl_dev, ctx->gl_dev + model->jeans_nodes)
+                 : build_universal<float>(ctx, ctx->gl_dev, ctx->gl_dev + model->jeans_nodes);
         if (rc != BANG_OK) break;
         if (cudaMalloc(&ctx->scal, 2 * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
+        if (cudaMalloc(&ctx->W_dev, ctx->W.size() * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
+        if (cudaMemcpyAsync(ctx->W_dev, ctx->W.data(), ctx->W.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess ||
+            cudaStreamSynchronize(ctx->stream) != cudaSuccess) { rc = BANG_ECUDA; break; }
+        rc = f64 ? setup_slow<double>(ctx) : setup_slow<float>(ctx);
+        if (rc != BANG_OK) break;
         // does the fused kernel fit (shared memory, registers)?
         FusedLaunch L = make_launch(ctx, nullptr, 1, 0, nullptr, nullptr);
         FusedInfo info{};
         cudaError_t e = dispatch_fused(ctx, L, &info, true);
         if (e != cudaSuccess) { rc = (e == cudaErrorInvalidValue || e == cudaErrorLaunchOutOfResources) ? BANG_EINVAL : BANG_ECUDA; break; }
     } while (0);
-    cudaFree(gl_dev);
     if (rc != BANG_OK) { cudaGetLastError(); bang_destroy(ctx); return rc; }
     *out = ctx;
     return BANG_OK;
@@ -538,9 +608,9 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
 int bang_set_data(bang_ctx* ctx, const double* data_dev, const double* err_dev, const unsigned char* mask_dev) {
     if (!ctx) return BANG_EINVAL;
     if (!data_dev || !err_dev || !mask_dev) return fail(ctx, BANG_EINVAL, "bang_set_data: null pointer");
-    CU(cudaSetDevice(ctx->device));
+    ON_DEVICE(ctx);
     double2* buf = nullptr;
-    const int gmax = (ctx->threads <= 128 ? 128 : (ctx->threads <= 256 ? 256 : 512)) / 4;      // lbc_threads / 4
+    const int gmax = data_gmax(ctx);
     const size_t n = (size_t)ctx->g.ny * 4 * ctx->P * gmax;
     CU(cudaMalloc(&buf, n * sizeof(double2)));
     CU(cudaMemsetAsync(buf, 0, n * sizeof(double2), ctx->stream));
@@ -564,14 +634,17 @@ int bang_model_maps(bang_ctx* ctx, const double* theta_dev, int B, void* maps_de
     if (!ctx) return BANG_EINVAL;
     if (B < 0 || (B > 0 && (!theta_dev || !maps_dev))) return fail(ctx, BANG_EINVAL, "bang_model_maps: bad arguments");
     if (B == 0) return BANG_OK;
-    CU(cudaSetDevice(ctx->device));
+    ON_DEVICE(ctx);
     if (ctx->model.psf_weighting == BANG_PSF_FLUX)
         return ctx->model.precision == BANG_FP64 ? run_flux<double>(ctx, theta_dev, B, 0, maps_dev, nullptr)
                                                  : run_flux<float>(ctx, theta_dev, B, 0, maps_dev, nullptr);
+    int rc = ensure_slow_list(ctx, B);
+    if (rc != BANG_OK) return rc;
     FusedLaunch L = make_launch(ctx, theta_dev, B, 0, maps_dev, nullptr);
     CU(dispatch_fused(ctx, L, nullptr, false));
     ctx->launches += 1;
-    return BANG_OK;
+    return ctx->model.precision == BANG_FP64 ? run_slow<double>(ctx, theta_dev, 0, maps_dev, nullptr)
+                                             : run_slow<float>(ctx, theta_dev, 0, maps_dev, nullptr);
 }
 
 int bang_loglike(bang_ctx* ctx, const double* theta_dev, int B, double* logL_dev) {
@@ -579,28 +652,32 @@ int bang_loglike(bang_ctx* ctx, const double* theta_dev, int B, double* logL_dev
     if (B < 0 || (B > 0 && (!theta_dev || !logL_dev))) return fail(ctx, BANG_EINVAL, "bang_loglike: bad arguments");
     if (!ctx->has_data) return fail(ctx, BANG_ENODATA, "bang_loglike: no data loaded");
     if (B == 0) return BANG_OK;
-    CU(cudaSetDevice(ctx->device));
+    ON_DEVICE(ctx);
     if (ctx->model.psf_weighting == BANG_PSF_FLUX)
         return ctx->model.precision == BANG_FP64 ? run_flux<double>(ctx, theta_dev, B, 1, nullptr, logL_dev)
                                                  : run_flux<float>(ctx, theta_dev, B, 1, nullptr, logL_dev);
+    int rc = ensure_slow_list(ctx, B);
+    if (rc != BANG_OK) return rc;
     FusedLaunch L = make_launch(ctx, theta_dev, B, 1, nullptr, logL_dev);
     CU(dispatch_fused(ctx, L, nullptr, false));
     ctx->launches += 1;
-    return BANG_OK;
+    return ctx->model.precision == BANG_FP64 ? run_slow<double>(ctx, theta_dev, 1, nullptr, logL_dev)
+                                             : run_slow<float>(ctx, theta_dev, 1, nullptr, logL_dev);
 }
 
 int bang_model_fine(bang_ctx* ctx, const double* theta_dev, int B, void* fine_dev) {
     if (!ctx) return BANG_EINVAL;
     if (B < 0 || (B > 0 && (!theta_dev || !fine_dev))) return fail(ctx, BANG_EINVAL, "bang_model_fine: bad arguments");
     if (B == 0) return BANG_OK;
-    CU(cudaSetDevice(ctx->device));
+    ON_DEVICE(ctx);
     const bool f64 = ctx->model.precision == BANG_FP64;
     const int ctas = std::min(B, 8 * ctx->n_sm);
+    const DirectC direct{ctx->gl_dev, ctx->gl_dev + ctx->model.jeans_nodes, ctx->model.jeans_nodes};
     if (f64) {
         FineParams<double> p{ctx->g, ctx->fit,
                              PolyTab<double>{static_cast<const double*>(ctx->btab), ctx->btab_first, ctx->btab_cells},
                              PolyTab<double>{static_cast<const double*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells},
-                             theta_dev, B, static_cast<double*>(fine_dev)};
+                             direct, theta_dev, B, static_cast<double*>(fine_dev)};
         const size_t smem = fused_smem_bytes<double>(0, 0);
         CU(cudaFuncSetAttribute(k_fine<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_fine<double><<<ctas, 256, smem, ctx->stream>>>(p);
@@ -608,7 +685,7 @@ int bang_model_fine(bang_ctx* ctx, const double* theta_dev, int B, void* fine_de
         FineParams<float> p{ctx->g, ctx->fit,
                             PolyTab<float>{static_cast<const float*>(ctx->btab), ctx->btab_first, ctx->btab_cells},
                             PolyTab<float>{static_cast<const float*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells},
-                            theta_dev, B, static_cast<float*>(fine_dev)};
+                            direct, theta_dev, B, static_cast<float*>(fine_dev)};
         const size_t smem = fused_smem_bytes<float>(0, 0);
         CU(cudaFuncSetAttribute(k_fine<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_fine<float><<<ctas, 256, smem, ctx->stream>>>(p);
@@ -623,7 +700,7 @@ int bang_loglike_host(bang_ctx* ctx, const double* theta_host, int B, double* lo
     if (B < 0 || (B > 0 && (!theta_host || !logL_host))) return fail(ctx, BANG_EINVAL, "bang_loglike_host: bad arguments");
     if (!ctx->has_data) return fail(ctx, BANG_ENODATA, "bang_loglike_host: no data loaded");
     if (B == 0) return BANG_OK;
-    CU(cudaSetDevice(ctx->device));
+    ON_DEVICE(ctx);
     int rc = ensure_staging(ctx, B, (size_t)B * sizeof(double));
     if (rc != BANG_OK) return rc;
     const size_t tb = (size_t)B * kNTheta * sizeof(double);
@@ -641,7 +718,7 @@ int bang_model_maps_host(bang_ctx* ctx, const double* theta_host, int B, void* m
     if (!ctx) return BANG_EINVAL;
     if (B < 0 || (B > 0 && (!theta_host || !maps_host))) return fail(ctx, BANG_EINVAL, "bang_model_maps_host: bad arguments");
     if (B == 0) return BANG_OK;
-    CU(cudaSetDevice(ctx->device));
+    ON_DEVICE(ctx);
     const size_t esz = ctx->model.precision == BANG_FP64 ? 8 : 4;
     const size_t ob = (size_t)B * 4 * ctx->g.nx * ctx->g.ny * esz;
     int rc = ensure_staging(ctx, B, ob);

@@ -38,12 +38,14 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
         info->regs = fa.numRegs; info->max_ctas_per_sm = per_sm; info->smem = smem; info->ctas = ctas;
     }
     if (query_only || L.B <= 0) return cudaSuccess;
+#ifdef BANG_TUNING
     if (getenv("BANG_VERBOSE")) {
         cudaFuncAttributes fa;
         cudaFuncGetAttributes(&fa, kern);
         fprintf(stderr, "[bang] k_fused<%s,S=%d,NACC=%d,P=%d,MODE=%d,LBC=%d> regs=%d smem=%zu threads=%d ctas/SM=%d grid=%d B=%d\n",
                 sizeof(T) == 4 ? "f32" : "f64", S, NACC, P, MODE, LBC, fa.numRegs, smem, L.threads, per_sm, ctas, L.B);
     }
+#endif
 
     FusedParams<T, S, NACC> p;
     p.g = L.g; p.fit = L.fit;
@@ -52,6 +54,7 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     for (int t = 0; t < NACC * S; ++t) p.W[t] = (T)L.W[t];
     p.theta = L.theta; p.B = L.B; p.nxp = L.nxp;
     p.maps = static_cast<T*>(L.maps); p.data = L.data; p.C0 = L.C0; p.logL = L.logL;
+    p.slow_list = L.slow_list; p.slow_count = L.slow_count;
     kern<<<ctas, L.threads, smem, L.stream>>>(p);
     return cudaGetLastError();
 }
@@ -70,6 +73,10 @@ cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
 
 template <typename T, int S, int P>
 cudaError_t launch_nacc(const FusedLaunch& L, FusedInfo* info, bool q) {
+#ifdef BANG_ONLY_NACC      // development builds: instantiate one accumulator depth only (seconds instead of minutes)
+    if (L.nacc == BANG_ONLY_NACC) return launch_one<T, S, BANG_ONLY_NACC, P>(L, info, q);
+    return cudaErrorInvalidValue;
+#else
     switch (L.nacc) {
         case 1: return launch_one<T, S, 1, P>(L, info, q);
         case 4: return launch_one<T, S, 4, P>(L, info, q);
@@ -78,6 +85,7 @@ cudaError_t launch_nacc(const FusedLaunch& L, FusedInfo* info, bool q) {
         case 13: return launch_one<T, S, 13, P>(L, info, q);
         default: return cudaErrorInvalidValue;
     }
+#endif
 }
 
 }  // namespace

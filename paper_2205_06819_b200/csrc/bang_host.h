@@ -19,6 +19,7 @@ struct FusedLaunch {
     const double2* data;
     double C0;
     double* logL;
+    int* slow_list; int* slow_count;   // theta left to the direct path (k_slow), see FusedParams
     int threads, ctas;           // launch shape (ctas = 0: let the launcher size a persistent grid)
     int n_sm;
     int* cache;                  // [2] resident CTAs per SM of the mode's kernel once configured (0 = not yet), or NULL

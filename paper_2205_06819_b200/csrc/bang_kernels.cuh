@@ -3,13 +3,22 @@
 // Step names are those of SURVEY.md sec. 8(a) / DESIGN.md "The path".  T = float (BANG_FP32) or double (BANG_FP64).
 #pragma once
 #include <cuda_runtime.h>
+#include <cstdio>
 
 #include "bang_math.cuh"
+
+// -DBANG_CHECK: a debug build whose kernels trap on a table index or a row-buffer offset out of range (the stand-in for
+// compute-sanitizer, which is closed on the GPU pool); the release build relies on decode_theta's range checks.
+#ifdef BANG_CHECK
+#define BANG_ASSERT(cond) do { if (!(cond)) { printf("BANG_CHECK failed: %s (%s:%d)\n", #cond, __FILE__, __LINE__); __trap(); } } while (0)
+#else
+#define BANG_ASSERT(cond) do { } while (0)
+#endif
 
 namespace bang {
 
 constexpr int kNTheta = 17;      // Table 1
-constexpr int kMaxOct = 64;          // octaves of r^2 the per-theta v_c table may span
+constexpr int kVcOct = 32;           // octaves of r^2 the per-theta v_c table holds (a theta that needs more takes the direct path)
 constexpr unsigned C_BULGE = 1u, C_DISC1 = 2u, C_DISC2 = 4u, C_HALO = 8u;
 constexpr int kBulgeOctLo = -44, kBulgeOctHi = 36;    // universal bulge tables: s^2 in [2^-44, 2^36)
 constexpr int kFOctLo = -60, kFOctHi = 10;            // universal Freeman table: y^2 in [2^-60, 2^10)
@@ -45,12 +54,16 @@ struct ThetaD {      // what the table build needs, in double
     double GMb, Rb;              // bulge v_c^2 = GMb r/(r+Rb)^2  (eq. 2)
     double Ad[2], inv2Rd[2];     // disc  v_c^2 = Ad F(r inv2Rd),  Ad = 2 G M_d/R_d  (eq. 9, reading D)
     double Ah, hs;               // halo: Hernquist GMh, Rh;  NFW: G M200/mu(c), 1/r_s  (reading H)
+    double ghc, ghs, gxp0, gyp0, gtan2i;   // the geometry of ThetaC (hc, hs, xp0, yp0, tan2i) in double: direct path
 };
 template <typename T>
 struct ThetaC {
-    int valid;
+    int valid;                   // 0: theta outside the model's domain (NaN maps, logL = -inf)
+    int slow;                    // 1: radii on this theta's grid leave the tabulated ranges -> direct evaluation per cell
     int jcx, jcy;                // fine cell (buffer coordinates) nearest to the galaxy centre
-    int vfirst, vcells;          // per-theta v_c table: first global interval, number of intervals
+    int vfirst, vcells;          // per-theta v_c table: first global interval, number of regular intervals (entry 0 of the
+                                 // table is the constant v_c of the cell nearest to the centre, entries 1.. the intervals)
+    T vc_near;                   // v_c at that cell
     T hc, hs;                    // h cos PA, h sin PA   (h = fine cell size in kpc)
     T xp0, yp0;                  // rotated offset of cell (jcx, jcy) from the centre
     T tan2i;                     // tan^2 i = 1/cos^2 i - 1
@@ -168,9 +181,10 @@ BANG_D float vc2_total_f(const ThetaF& d, const GridC& g, const PolyTab<float>& 
 
 // a0: decode theta[17] (Table 1).  Run by ONE thread; everything in fp64.
 template <typename T>
-BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, ThetaC<T>& c) {
+BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, const PolyTab<T>& Ftab, ThetaC<T>& c) {
     const unsigned comps = g.comps;
     c.valid = 0;
+    c.slow = 0;
     bool ok = isfinite(th[0]) && isfinite(th[1]) && isfinite(th[2]) && isfinite(th[3]) && fabs(th[3]) < 90.0;
     if (comps & C_BULGE) ok = ok && isfinite(th[4]) && th[5] > 0 && isfinite(th[5]) && th[12] > 0 && isfinite(th[12]);
     for (int j = 0; j < 2; ++j)
@@ -191,12 +205,19 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, ThetaC<T
     const double dx = (jcx - Jsx) * h, dy = (jcy - Jsy) * h;                    // offset of that cell from the centre [kpc]
     c.jcx = jcx; c.jcy = jcy;
     c.hc = (T)(h * cp); c.hs = (T)(h * sp);
-    c.xp0 = (T)(dx * cp + dy * sp);
-    c.yp0 = (T)(-dx * sp + dy * cp);
+    const double xp0 = dx * cp + dy * sp, yp0 = -dx * sp + dy * cp;
+    c.xp0 = (T)xp0;
+    c.yp0 = (T)yp0;
     const double inv_ci2 = 1.0 / (ci * ci);
-    c.tan2i = (T)((si * si) / (ci * ci));
+    const double tan2i = (si * si) / (ci * ci);
+    c.tan2i = (T)tan2i;
+    c.d.ghc = h * cp; c.d.ghs = h * sp; c.d.gxp0 = xp0; c.d.gyp0 = yp0; c.d.gtan2i = tan2i;
 
-    // range of radii on this theta's grid: R^2 >= dx^2+dy^2 (attained at the nearest cell); maxima at the corners
+    // Range of radii on this theta's grid.  R^2 is smallest at the cell nearest to the centre (R2min); every OTHER cell
+    // of the lattice has R^2 >= h^2/4 when the centre lies inside that cell, >= R2min when it lies outside the grid.
+    // Maxima at the corners.  The per-theta v_c table covers [Llo, r2max] with its regular intervals and serves the
+    // nearest cell with a dedicated constant entry, so that a centre that falls on (or next to) a cell centre does not
+    // cost tens of empty octaves.
     const double floor2 = ldexp(1.0, 2 * kRFloorLog2);
     const double R2min = fmax(dx * dx + dy * dy, floor2);
     double R2max = 0.0, r2max = 0.0;
@@ -209,10 +230,15 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, ThetaC<T
     }
     R2max = fmax(R2max, floor2); r2max = fmax(r2max, floor2);
     const double lo_m = 1.0 - 0x1p-10, hi_m = 1.0 + 0x1p-10;
-    const int e_lo = ilogb(R2min * lo_m), e_hi = ilogb(r2max * hi_m);
-    if (e_hi - e_lo + 1 > kMaxOct || e_hi > 120) return;
+    const bool inside = fabs(dx) <= 0.5 * h * hi_m && fabs(dy) <= 0.5 * h * hi_m;
+    const double Llo = inside ? fmin(0.25 * h * h, r2max) : R2min;
+    const int e_lo = ilogb(Llo * lo_m), e_hi = ilogb(r2max * hi_m);
+    if (e_hi - e_lo + 1 > kVcOct || e_hi > 100) c.slow = 1;                      // direct evaluation (eval_cell_direct)
+    // fp32 mode: r^2 = R^2 + y'^2 tan^2 i amplifies the rounding of y' (relative ~2^-23 per operation) by tan i; beyond
+    // tan i = 64 (i > 89.1 deg) that approaches the mode's 1e-4, so such theta take the direct path (fp64 geometry)
+    if (sizeof(T) == 4 && tan2i > 4096.0) c.slow = 1;
     c.vfirst = tab_first_cell<T>(e_lo);
-    c.vcells = (e_hi - e_lo + 1) << TabCfg<T>::M;
+    c.vcells = c.slow ? 0 : (e_hi - e_lo + 1) << TabCfg<T>::M;
 
     ThetaD& d = c.d;
     // bulge: eq. 1-6
@@ -221,7 +247,8 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, ThetaC<T
     if (comps & C_BULGE) {      // eq. 1-6 (Hernquist) or App. B (Jaffe): both scale-free in s = R/R_b
         const double Mb = exp10(th[4]), Rb = th[5], MLb = th[12];
         const double inv = 1.0 / (Rb * Rb);
-        if (!(R2min * inv * lo_m >= ldexp(1.0, kBulgeOctLo)) || !(R2max * inv * hi_m < ldexp(1.0, kBulgeOctHi))) return;
+        // s^2 = R^2/R_b^2 must stay inside the scale-free tables; otherwise the direct path evaluates eq. 4-6 per cell
+        if (!(R2min * inv * lo_m >= ldexp(1.0, kBulgeOctLo)) || !(R2max * inv * hi_m < ldexp(1.0, kBulgeOctHi))) c.slow = 1;
         c.invRb2 = (T)inv;
         if (g.bulge_profile == 1) {
             c.ampBb = (T)(Mb / (Rb * Rb) / MLb * 1e-6);                                  // eq. B4, in Lsun/pc^2
@@ -261,16 +288,21 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, ThetaC<T
             d.Ah = kG * Mh; d.hs = th[11];
         }
     }
+    // v_c at the cell nearest to the centre (entry 0 of the per-theta table)
+    c.vc_near = (T)sqrt(vc2_total<T>(d, g, Ftab, sqrt(R2min + yp0 * yp0 * tan2i)));
     c.valid = 1;
 }
 
 // a1: the per-theta radial table v_c(r), a piecewise polynomial in u = r^2 on the pseudo-log grid, built cooperatively
-// by the CTA in shared memory: every thread evaluates v_c at Chebyshev nodes (fp64), then one thread per interval turns
-// its D+1 node values into monomial coefficients.  Must be called by all threads; ends with a __syncthreads().
+// by the CTA in shared memory: every thread evaluates v_c at Chebyshev nodes, then one thread per interval turns its D+1
+// node values into monomial coefficients.  Entry 0 is the constant v_c of the cell nearest to the centre; the regular
+// intervals follow.  Must be called by all threads; ends with a __syncthreads().
 template <typename T>
 BANG_D void build_vc_table(const ThetaC<T>& c, const GridC& g, const FitC& fit, const PolyTab<T>& Ftab, T* vtab) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     const int n = c.vcells * NC;
+    if (threadIdx.x < NC) vtab[threadIdx.x] = threadIdx.x == 0 ? c.vc_near : T(0);
+    T* reg = vtab + NC;
     if constexpr (sizeof(T) == 4) {
         const ThetaF df{(float)c.d.GMb, (float)c.d.Rb, {(float)c.d.Ad[0], (float)c.d.Ad[1]},
                         {(float)c.d.inv2Rd[0], (float)c.d.inv2Rd[1]}, (float)c.d.Ah, (float)c.d.hs};
@@ -279,7 +311,7 @@ BANG_D void build_vc_table(const ThetaC<T>& c, const GridC& g, const FitC& fit, 
             double lo, width;
             tab_interval<T>(c.vfirst + cell, lo, width);
             const float u = (float)(lo + 0.5 * width * (fit.tnode[k] + 1.0));
-            vtab[i] = sqrtf(vc2_total_f(df, g, Ftab, sqrtf(u)));
+            reg[i] = sqrtf(vc2_total_f(df, g, Ftab, sqrtf(u)));
         }
     } else {
         for (int i = threadIdx.x; i < n; i += blockDim.x) {
@@ -287,12 +319,12 @@ BANG_D void build_vc_table(const ThetaC<T>& c, const GridC& g, const FitC& fit, 
             double lo, width;
             tab_interval<T>(c.vfirst + cell, lo, width);
             const double u = lo + 0.5 * width * (fit.tnode[k] + 1.0);
-            vtab[i] = (T)sqrt(vc2_total(c.d, g, Ftab, sqrt(u)));
+            reg[i] = (T)sqrt(vc2_total(c.d, g, Ftab, sqrt(u)));
         }
     }
     __syncthreads();
     for (int cell = threadIdx.x; cell < c.vcells; cell += blockDim.x) {
-        T* p = vtab + cell * NC;
+        T* p = reg + cell * NC;
         double f[NC], co[NC];
 #pragma unroll
         for (int k = 0; k < NC; ++k) f[k] = (double)p[k];
@@ -309,11 +341,13 @@ BANG_D void build_vc_table(const ThetaC<T>& c, const GridC& g, const FitC& fit, 
     __syncthreads();
 }
 
-// per-theta constants of the fine-cell model, copied from shared memory into registers once per theta so that the
-// per-cell code below touches shared memory only for its table look-up
+// per-theta constants of the fine-cell model, copied from shared memory into registers so that the per-cell code below
+// touches shared memory only for its table look-up
 template <typename T>
 struct CellK {
-    int jcx, jcy, vfirst, vlast;
+    int jcx, jcy;
+    int vfirst1;                 // global interval number of table entry 0 (= first regular interval - 1)
+    int vlast;                   // last valid entry (BANG_CHECK builds only)
     T hc, hs, xp0, yp0, tan2i;
     T invRb2, ampBb, ampIb, MLb;
     T cexp0, cexp1, ampBd0, ampBd1, ampSd0, ampSd1, vkB0, vkB1, q3B0, q3B1;
@@ -321,7 +355,7 @@ struct CellK {
 template <typename T>
 BANG_D CellK<T> load_cellk(const ThetaC<T>& c) {
     CellK<T> k;
-    k.jcx = c.jcx; k.jcy = c.jcy; k.vfirst = c.vfirst; k.vlast = c.vcells - 1;
+    k.jcx = c.jcx; k.jcy = c.jcy; k.vfirst1 = c.vfirst - 1; k.vlast = c.vcells;
     k.hc = c.hc; k.hs = c.hs; k.xp0 = c.xp0; k.yp0 = c.yp0; k.tan2i = c.tan2i;
     k.invRb2 = c.invRb2; k.ampBb = c.ampBb; k.ampIb = c.ampIb; k.MLb = c.MLb;
     k.cexp0 = c.cexp[0]; k.cexp1 = c.cexp[1]; k.ampBd0 = c.ampBd[0]; k.ampBd1 = c.ampBd[1];
@@ -337,12 +371,37 @@ BANG_D void rotate_cell(const CellK<T>& k, const T a, const T b, T& xp, T& yp) {
     yp = fma(b, k.hc, fma(-a, k.hs, k.yp0));
 }
 
-// a2 + a3: one fine cell at (xp, yp) in the galaxy frame -> B_tot, v_los, sigma_los, <L/M>   (eqs. 4-15, 19).  BULGE: the model has a bulge; SHIFT = 0/1/2/3: without a bulge
-// the disc exponentials are scaled by disc 1 (1), disc 2 (2) or the larger of the two (3) so that the ratios below
-// survive fp32 underflow far outside small discs.
+// eq. 13, 14 (with 11), 15 (with 12), 19 from the per-cell ingredients: bulge light Bb and Bb sigma_b^2 (IbL), the disc
+// exponentials E1, E2 (scaled by 2^-shift without a bulge), v_c and cos(phi).  FLUX: reading G' (light moments).
+template <typename T, bool BULGE, bool FLUX>
+BANG_D void combine_cell(const CellK<T>& k, const T Bb, const T IbL, const T E1, const T E2, const T shift, const T vc,
+                         const T cosphi, T& oB, T& oV, T& oS, T& oLM) {
+    const T Btot = fma(k.ampBd0, E1, fma(k.ampBd1, E2, Bb));
+    const T Stot = fma(k.ampSd0, E1, fma(k.ampSd1, E2, k.MLb * Bb));       // total mass surface density (x 1e-6)
+    const T invB = fast_rcp(Btot);
+    const T kB = fma(k.vkB0, E1, k.vkB1 * E2);                              // sum_j B_d,j (-k_j sin i)
+    const T qB = fma(k.q3B0, E1, k.q3B1 * E2);                              // sum_j B_d,j (1 - k_j^2)/3
+    oV = cosphi * vc * kB * invB;
+    oS = fast_sqrt(fma(vc * vc, qB, IbL) * invB);
+    oLM = Btot * fast_rcp(Stot);
+    oB = BULGE ? Btot : Btot * fast_exp2(shift);
+    if constexpr (FLUX) {
+        // reading G': the PSF acts on the light moments B, B v, B (sigma^2 + v^2) and on the mass surface density B / <L/M>
+        const T v = oV;
+        oV = oB * v;
+        oS = oB * fma(oS, oS, v * v);
+        oLM = oB * fast_rcp(oLM);
+    }
+}
+
+// a2 + a3: one fine cell at (xp, yp) in the galaxy frame -> B_tot, v_los, sigma_los, <L/M>   (eqs. 4-15, 19).  BULGE: the
+// model has a bulge; SHIFT = 0/1/2/3: without a bulge the disc exponentials are scaled by disc 1 (1), disc 2 (2) or the
+// larger of the two (3) so that the ratios below survive fp32 underflow far outside small discs.
+// bbase: the scale-free bulge table with its first interval folded in (coef - first * 2 (D+1)); the caller guarantees
+// that s^2 and r^2 stay inside the tables (decode_theta: otherwise the theta takes eval_cell_direct).
 template <typename T, bool BULGE, int SHIFT, bool FLUX = false>
-BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int bfirst, const int blast,
-                      const T* __restrict__ vtab, const T xp, const T yp, T& oB, T& oV, T& oS, T& oLM) {
+BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab, const T xp, const T yp,
+                      T& oB, T& oV, T& oS, T& oLM) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     // (xp, yp): the cell in the galaxy frame; R on the sky (bulge), r in the disc plane
     const T floor2 = sizeof(T) == 4 ? T(0x1p-32f) : T(0x1p-32);
@@ -359,8 +418,8 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int 
     T Bb = T(0), IbL = T(0);
     if constexpr (BULGE) {
         T t;
-        const int cell = (int)min((unsigned)(tab_cell(R2 * k.invRb2, t) - bfirst), (unsigned)blast);
-        const T* p = bcoef + (size_t)cell * (2 * NC);
+        const int cell = tab_cell(R2 * k.invRb2, t);
+        const T* p = bbase + (ptrdiff_t)cell * (2 * NC);
         T cs[NC], cj[NC];
         if constexpr (sizeof(T) == 4) {
             const float4 v0 = __ldg(reinterpret_cast<const float4*>(p));
@@ -383,11 +442,12 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int 
     T shift = T(0);
     if constexpr (!BULGE) shift = SHIFT == 1 ? e1a : (SHIFT == 2 ? e2a : fmax(e1a, e2a));
     const T E1 = fast_exp2(e1a - shift), E2 = fast_exp2(e2a - shift);     // B_d,j = ampBd_j E_j
-    // v_c(r) from the per-theta table (eq. 10)
+    // v_c(r) from the per-theta table (eq. 10); entry 0 serves the cell nearest to the centre
     T vc;
     {
         T t;
-        const int cell = (int)min((unsigned)(tab_cell(r2, t) - k.vfirst), (unsigned)k.vlast);
+        const int cell = max(tab_cell(r2, t) - k.vfirst1, 0);
+        BANG_ASSERT(cell <= k.vlast);
         const T* p = vtab + cell * NC;
         T cv[NC];
         if constexpr (sizeof(T) == 4) {
@@ -402,28 +462,68 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bcoef, const int 
         }
         vc = horner<T, D>(cv, t);
     }
-    // eq. 13, 14 (with 11), 15 (with 12), 19
-    const T Btot = fma(k.ampBd0, E1, fma(k.ampBd1, E2, Bb));
-    const T Stot = fma(k.ampSd0, E1, fma(k.ampSd1, E2, k.MLb * Bb));       // total mass surface density (x 1e-6)
-    const T invB = fast_rcp(Btot);
-    const T kB = fma(k.vkB0, E1, k.vkB1 * E2);                              // sum_j B_d,j (-k_j sin i)
-    const T qB = fma(k.q3B0, E1, k.q3B1 * E2);                              // sum_j B_d,j (1 - k_j^2)/3
-    oV = cosphi * vc * kB * invB;
-    oS = fast_sqrt(fma(vc * vc, qB, IbL) * invB);
-    oLM = Btot * fast_rcp(Stot);
-    oB = BULGE ? Btot : Btot * fast_exp2(shift);
-    if constexpr (FLUX) {
-        // reading G': the PSF acts on the light moments B, B v, B (sigma^2 + v^2) and on the mass surface density
-        // B / <L/M>; formed from the finished observables (k_fine only: the fused kernel never instantiates this)
-        const T v = oV;
-        oV = oB * v;
-        oS = oB * fma(oS, oS, v * v);
-        oLM = oB * fast_rcp(oLM);
-    }
+    combine_cell<T, BULGE, FLUX>(k, Bb, IbL, E1, E2, shift, vc, cosphi, oB, oV, oS, oLM);
 }
 
-// a2 + a3 over a run of whole fine rows: cells i = tid, tid + NT, ... of the n_rows x nfx block that starts at fine row
-// jy0, written to dst[row * row_pitch + observable * obs_stride + x].  All threads of the CTA take part.
+// The direct path: one fine cell evaluated without the per-theta table and, where s^2 leaves the scale-free tables,
+// without those either -- eq. 4-5 in closed form, eq. 6 by the N_J-node rule, eq. 10 term by term, in fp64.  Taken by the
+// rare theta whose grid spans more octaves of r^2 than the v_c table holds (|i| -> 90 deg) or whose R/R_b leaves
+// [2^-22, 2^18): the library's domain is the model's, not the tables'.  ~1e3-1e4 times slower per cell than eval_cell.
+struct DirectC {
+    const double* glx; const double* glw; int NJ;   // the Gauss-Legendre rule of reading B (device memory)
+};
+template <typename T, bool FLUX>
+__device__ __noinline__ void eval_cell_direct(const ThetaC<T>& c, const GridC& g, const PolyTab<T>& btab, const PolyTab<T>& Ftab,
+                                              const DirectC dc, const int a, const int b, T* o4) {
+    // (a, b): offsets in cells from the cell nearest to the centre; the geometry in fp64 whatever the mode (at |i| -> 90
+    // deg, r^2 = R^2 + y'^2 tan^2 i amplifies the rounding of fp32 coordinates beyond the mode's tolerance)
+    const double xp = (double)a * c.d.ghc + ((double)b * c.d.ghs + c.d.gxp0);
+    const double yp = (double)b * c.d.ghc + (c.d.gyp0 - (double)a * c.d.ghs);
+    const double y2 = yp * yp;
+    const double R2 = fmax(xp * xp + y2, 0x1p-32);
+    const double r2 = R2 + y2 * c.d.gtan2i;
+    const double r = sqrt(r2), cosphi = xp / r;
+    double Bb = 0.0, IbL = 0.0;
+    if (g.comps & C_BULGE) {
+        const double s2 = R2 * (double)c.invRb2;
+        double st, jj;
+        if (s2 >= ldexp(1.0, kBulgeOctLo) * (1.0 + 0x1p-9) && s2 < ldexp(1.0, kBulgeOctHi) * (1.0 - 0x1p-9)) {
+            T t;
+            const int cell = tab_cell((T)s2, t) - btab.first;
+            const T* p = btab.coef + (size_t)cell * (2 * (TabCfg<T>::D + 1));
+            st = (double)horner<T, TabCfg<T>::D>(p, t);
+            jj = (double)horner<T, TabCfg<T>::D>(p + TabCfg<T>::D + 1, t);
+        } else {
+            const double sx = sqrt(s2);
+            st = g.bulge_profile == 1 ? jaffe_sigma_tilde(sx) : sigma_tilde(sx);
+            jj = g.bulge_profile == 1 ? jaffe_jeans_J(sx, dc.NJ, dc.glx, dc.glw) : jeans_J(sx, dc.NJ, dc.glx, dc.glw);
+        }
+        Bb = (double)c.ampBb * st;
+        IbL = (double)c.ampIb * jj;
+    }
+    const double vc2 = vc2_total<T>(c.d, g, Ftab, r);
+    // discs, with the common factor 2^shift taken out of the exponentials (no bulge: the ratios survive underflow)
+    const double e1a = r * (double)c.cexp[0], e2a = r * (double)c.cexp[1];
+    double shift = 0.0;
+    if (!(g.comps & C_BULGE)) {
+        const bool d1 = g.comps & C_DISC1, d2 = g.comps & C_DISC2;
+        shift = (d1 && d2) ? fmax(e1a, e2a) : (d1 ? e1a : e2a);
+    }
+    const double E1 = exp2(e1a - shift), E2 = exp2(e2a - shift);
+    const double Btot = (double)c.ampBd[0] * E1 + (double)c.ampBd[1] * E2 + Bb;
+    const double Stot = (double)c.ampSd[0] * E1 + (double)c.ampSd[1] * E2 + (double)c.MLb * Bb;
+    const double kB = (double)c.vkB[0] * E1 + (double)c.vkB[1] * E2;
+    const double qB = (double)c.q3B[0] * E1 + (double)c.q3B[1] * E2;
+    double oB = Btot * exp2(shift), oV = cosphi * sqrt(vc2) * kB / Btot, oS = sqrt((vc2 * qB + IbL) / Btot), oLM = Btot / Stot;
+    if (FLUX) {
+        const double v = oV;
+        oV = oB * v; oS = oB * (oS * oS + v * v); oLM = oB / oLM;
+    }
+    o4[0] = (T)oB; o4[1] = (T)oV; o4[2] = (T)oS; o4[3] = (T)oLM;
+}
+
+// a2 + a3 over a run of whole fine rows (k_fine): cells i = tid, tid + NT, ... of the n_rows x nfx block that starts at
+// fine row jy0, written to dst[row * row_pitch + observable * obs_stride + x].  All threads of the CTA take part.
 struct EvalWalk { int i0, j0, x0, step_j, step_x; };   // flat cell i = i0 + n NT sits at (row j, column x)
 BANG_D EvalWalk make_walk(const int tid, const int NT, const int nfx) {
     EvalWalk w;
@@ -432,19 +532,17 @@ BANG_D EvalWalk make_walk(const int tid, const int NT, const int nfx) {
     return w;
 }
 template <typename T, bool BULGE, int SHIFT, bool FLUX>
-BANG_D void eval_rows(const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab, T* __restrict__ dst,
+BANG_D void eval_rows(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab, T* __restrict__ dst,
                       const size_t row_pitch, const size_t obs_stride, const int nfx, const int jy0, const int n_rows,
                       const EvalWalk& w, const int NT) {
     const int step_j = w.step_j, step_x = w.step_x;
     int j = w.j0, x = w.x0;
     const int tid = w.i0;
     const int n = n_rows * nfx;
-    const T* __restrict__ bcoef = btab.coef;
-    const int bfirst = btab.first, blast = btab.n_cells - 1;
     for (int i = tid; i < n; i += NT) {
         T vB, vV, vS, vL, xp, yp;
         rotate_cell<T>(k, (T)(x - k.jcx), (T)(jy0 + j - k.jcy), xp, yp);
-        eval_cell<T, BULGE, SHIFT, FLUX>(k, bcoef, bfirst, blast, vtab, xp, yp, vB, vV, vS, vL);
+        eval_cell<T, BULGE, SHIFT, FLUX>(k, bbase, vtab, xp, yp, vB, vV, vS, vL);
         T* d = dst + (size_t)j * row_pitch + x;
         d[0] = vB; d[obs_stride] = vV; d[2 * obs_stride] = vS; d[3 * obs_stride] = vL;
         x += step_x; j += step_j;
@@ -452,39 +550,82 @@ BANG_D void eval_rows(const CellK<T>& k, const PolyTab<T>& btab, const T* __rest
     }
 }
 template <typename T, bool FLUX>
-BANG_D void eval_rows_comps(const unsigned comps, const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab,
+BANG_D void eval_rows_comps(const unsigned comps, const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab,
                             T* __restrict__ dst, const size_t row_pitch, const size_t obs_stride, const int nfx,
                             const int jy0, const int n_rows, const EvalWalk& w, const int NT) {
-    if (comps & C_BULGE) eval_rows<T, true, 0, FLUX>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    if (comps & C_BULGE) eval_rows<T, true, 0, FLUX>(k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_rows<T, false, 3, FLUX>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
-    else if (comps & C_DISC1) eval_rows<T, false, 1, FLUX>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
-    else eval_rows<T, false, 2, FLUX>(k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+        eval_rows<T, false, 3, FLUX>(k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else if (comps & C_DISC1) eval_rows<T, false, 1, FLUX>(k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else eval_rows<T, false, 2, FLUX>(k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
 }
 template <typename T>
-BANG_D void eval_rows_any(const unsigned comps, const bool flux, const CellK<T>& k, const PolyTab<T>& btab,
+BANG_D void eval_rows_any(const unsigned comps, const bool flux, const CellK<T>& k, const T* __restrict__ bbase,
                           const T* __restrict__ vtab, T* __restrict__ dst, const size_t row_pitch, const size_t obs_stride,
                           const int nfx, const int jy0, const int n_rows, const EvalWalk& w, const int NT) {
-    if (flux) eval_rows_comps<T, true>(comps, k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
-    else eval_rows_comps<T, false>(comps, k, btab, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    if (flux) eval_rows_comps<T, true>(comps, k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else eval_rows_comps<T, false>(comps, k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+}
+// the same block of rows through the direct path (a theta flagged slow)
+template <typename T>
+BANG_D void eval_rows_direct(const bool flux, const ThetaC<T>& c, const GridC& g, const PolyTab<T>& btab, const PolyTab<T>& Ftab,
+                             const DirectC dc, const CellK<T>& k, T* __restrict__ dst, const size_t row_pitch,
+                             const size_t obs_stride, const int nfx, const int jy0, const int n_rows, const int tid, const int NT) {
+    const int n = n_rows * nfx;
+    for (int i = tid; i < n; i += NT) {
+        const int j = i / nfx, x = i - j * nfx;
+        T o[4];
+        if (flux) eval_cell_direct<T, true>(c, g, btab, Ftab, dc, x - k.jcx, jy0 + j - k.jcy, o);
+        else eval_cell_direct<T, false>(c, g, btab, Ftab, dc, x - k.jcx, jy0 + j - k.jcy, o);
+        T* d = dst + (size_t)j * row_pitch + x;
+        d[0] = o[0]; d[obs_stride] = o[1]; d[2 * obs_stride] = o[2]; d[3 * obs_stride] = o[3];
+    }
+}
+
+// ---- row buffer geometry --------------------------------------------------------------------------------------------
+// The fused kernel keeps one super-row (S fine rows x 4 observables) in shared memory: plane (j, q) at (j 4 + q) NFB,
+// cell x of a plane at x + PADV (x / GRP).  NFB, the plane pitch in cells, is a compile-time constant of the
+// instantiation (immediate store offsets): the widest row the launch-bound class can hold.
+// Bank conflicts.  In the PSF phase neighbouring threads read 16-byte vectors GRP = P S cells apart.  When that stride is
+// an EVEN number of vectors (s = 4 with P = 4: 64 B), the 8 lanes of a quarter-warp fall on 2 or 4 of the 8 vector-wide
+// bank groups (ncu, config 5: 7 conflicts per load); one pad vector after every GRP cells makes the stride odd and the
+// loads conflict-free.  row_pad = pad cells per group (0 when not needed).
+constexpr int row_pad(int P, int S, int elem_bytes) {
+    const int V = 16 / elem_bytes, GRP = P * S;
+    return (GRP % V == 0 && (GRP / V) % 2 == 0) ? V : 0;
+}
+// LBC: launch-bound class = the CTA-size bracket the kernel is compiled for, which fixes its register budget, the
+// row-buffer pitch (hence the shared memory per CTA) and the pitch of the data array:
+//   0: <= 128 threads, 7 (P = 2) or 6 (P = 4) CTAs per SM;  1: <= 256 threads, 3 or 2 CTAs per SM;  2: <= 512 threads
+//   (2 CTAs per SM with P = 2, else 1).
+constexpr int lbc_threads(int lbc) { return lbc == 0 ? 128 : (lbc == 1 ? 256 : 512); }
+// plane pitch: nxp <= threads P / 4 data columns, i.e. (nxp - 1 + NACC) S cells, rounded up to a multiple of 4, plus 4
+// cells of over-read slack for the vector loads
+constexpr int lbc_nfb(int lbc, int P, int S, int NACC, int elem_bytes) {
+    const int cells = (lbc_threads(lbc) * P / 4 - 1 + NACC) * S;
+    const int padded = cells + row_pad(P, S, elem_bytes) * ((cells + P * S - 1) / (P * S));
+    return (padded + 3) / 4 * 4 + 4 + row_pad(P, S, elem_bytes);
+}
+constexpr int lbc_blocks(int lbc, int P, bool f64) {
+    return f64 ? (lbc == 0 ? 4 : (lbc == 1 ? 2 : 1))          // fp64 mode: 128 registers in every class
+               : (lbc == 0 ? (P == 2 ? 7 : 6) : (lbc == 1 ? (P == 2 ? 3 : 2) : (P == 2 ? 2 : 1)));
 }
 
 // a2 + a3 for one super-row of the fused kernel (S fine rows jy0 .. jy0+S-1 = one data row): thread `vt` takes the fine
 // columns x = vt, vt + NT, ... and evaluates the S cells of each column in one iteration, so that the index arithmetic,
 // the rotation and the store address are shared by S cells and S independent dependency chains are in flight.
-// dst[(row * 4 + observable) * NFB + x] (NFB, the plane pitch, is a compile-time constant: immediate store offsets).  GUARD: some of the S rows lie past the grid (zero-weight tap padding): they are
-// written as zeros.
+// dst[(row * 4 + observable) * NFB + x].  GUARD: some of the S rows lie past the grid (zero-weight tap padding): they
+// are written as zeros.
 template <typename T, int S, int NFB, int GRP, int PADV, bool BULGE, int SHIFT, bool GUARD>
-BANG_D void eval_superrow(const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab, T* __restrict__ dst,
+BANG_D void eval_superrow(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab, T* __restrict__ dst,
                           const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
-    const T* __restrict__ bcoef = btab.coef;
-    const int bfirst = btab.first, blast = btab.n_cells - 1;
     const T b0 = (T)(jy0 - k.jcy);
     const T bx = fma(b0, k.hs, k.xp0), by = fma(b0, k.hc, k.yp0);
     for (int x = vt; x < nfx; x += NT) {
         const T a = (T)(x - k.jcx);
         const T px = fma(a, k.hc, bx), py = fma(-a, k.hs, by);
         T* d = dst + x + (PADV ? PADV * (x / GRP) : 0);      // row_pad: GRP is a power of two whenever PADV != 0
+        BANG_ASSERT(x + (PADV ? PADV * (x / GRP) : 0) < NFB);
 #pragma unroll
         for (int j = 0; j < S; ++j) {
             T vB, vV, vS, vL;
@@ -492,21 +633,20 @@ BANG_D void eval_superrow(const CellK<T>& k, const PolyTab<T>& btab, const T* __
                 vB = vV = vS = vL = T(0);
             } else {
                 const T xp = j == 0 ? px : fma((T)j, k.hs, px), yp = j == 0 ? py : fma((T)j, k.hc, py);
-                eval_cell<T, BULGE, SHIFT>(k, bcoef, bfirst, blast, vtab, xp, yp, vB, vV, vS, vL);
+                eval_cell<T, BULGE, SHIFT>(k, bbase, vtab, xp, yp, vB, vV, vS, vL);
             }
             d[(j * 4 + 0) * NFB] = vB; d[(j * 4 + 1) * NFB] = vV; d[(j * 4 + 2) * NFB] = vS; d[(j * 4 + 3) * NFB] = vL;
         }
     }
 }
 template <typename T, int S, int NFB, int GRP, int PADV, bool GUARD>
-BANG_D void eval_superrow_any(const unsigned comps, const CellK<T>& k, const PolyTab<T>& btab, const T* __restrict__ vtab,
-                              T* __restrict__ dst, const int nfx, const int nfy, const int jy0,
-                              const int vt, const int NT) {
-    if (comps & C_BULGE) eval_superrow<T, S, NFB, GRP, PADV, true, 0, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
+BANG_D void eval_superrow_any(const unsigned comps, const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab,
+                              T* __restrict__ dst, const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
+    if (comps & C_BULGE) eval_superrow<T, S, NFB, GRP, PADV, true, 0, GUARD>(k, bbase, vtab, dst, nfx, nfy, jy0, vt, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_superrow<T, S, NFB, GRP, PADV, false, 3, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else if (comps & C_DISC1) eval_superrow<T, S, NFB, GRP, PADV, false, 1, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else eval_superrow<T, S, NFB, GRP, PADV, false, 2, GUARD>(k, btab, vtab, dst, nfx, nfy, jy0, vt, NT);
+        eval_superrow<T, S, NFB, GRP, PADV, false, 3, GUARD>(k, bbase, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else if (comps & C_DISC1) eval_superrow<T, S, NFB, GRP, PADV, false, 1, GUARD>(k, bbase, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else eval_superrow<T, S, NFB, GRP, PADV, false, 2, GUARD>(k, bbase, vtab, dst, nfx, nfy, jy0, vt, NT);
 }
 
 // ---- the fused kernel ---------------------------------------------------------------------------------------------
@@ -524,17 +664,20 @@ struct FusedParams {
                                  // (thread class of the launch) / 4 >= nxp/P
     double C0;                   // sum over used pixels of -1/2 ln(2 pi e^2)
     double* logL;                // [B]
+    int* slow_list;              // [>= B] indices of the theta that need the direct path (k_slow, bang_slow.cuh) ...
+    int* slow_count;             // ... and their number; NULL: such theta are reported as out of domain
 };
 
 template <typename T>
+inline size_t vtab_bytes() { return ((size_t)kVcOct * (1 << TabCfg<T>::M) + 1) * (TabCfg<T>::D + 1) * sizeof(T); }
+template <typename T>
 inline size_t fused_smem_bytes(int S, int nfb) {
-    return (sizeof(ThetaC<T>) + 15) / 16 * 16 + (size_t)kMaxOct * (1 << TabCfg<T>::M) * (TabCfg<T>::D + 1) * sizeof(T) +
-           (size_t)S * 4 * nfb * sizeof(T) + 32 * sizeof(double);
+    return (sizeof(ThetaC<T>) + 15) / 16 * 16 + vtab_bytes<T>() + (size_t)S * 4 * nfb * sizeof(T) + 32 * sizeof(double);
 }
 
 // N consecutive values from shared memory into registers with the widest vector loads the alignment ALIGN (bytes)
 // allows; may read up to one vector past N (the row buffer carries that slack).
-// GRP, PADV: the buffer holds PADV pad elements after every GRP elements (row_pad below); src points at a group start.
+// GRP, PADV: the buffer holds PADV pad elements after every GRP elements (row_pad above); src points at a group start.
 template <typename T, int N, int ALIGN, int GRP, int PADV>
 BANG_D void load_run(const T* __restrict__ src, T (&f)[N]) {
     constexpr int V = ALIGN / (int)sizeof(T);
@@ -568,37 +711,11 @@ BANG_D void load_run(const T* __restrict__ src, T (&f)[N]) {
 }
 
 // 1/x for the final M/L = 1/<L/M> (fn 10): MUFU.RCP (1 ulp) in fp32 mode, IEEE division in fp64 mode
-// The argument is floored far below any physical <L/M> so that padded pixels (accumulators = 0) stay finite and drop
-// out of the chi-square through their weight 1/e = 0 without a per-pixel guard.
+// The argument is floored far below any physical <L/M> so that padded pixels (accumulators = 0) stay finite.
 BANG_D float inv_ml(float x) { return fast_rcp(fmaxf(x, 1e-30f)); }
 BANG_D double inv_ml(double x) { return 1.0 / fmax(x, 1e-300); }
 
 // MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike)
-// LBC: launch-bound class = the CTA-size bracket the kernel is compiled for, which fixes its register budget:
-//   0: <= 128 threads, 7 (P = 2) or 6 (P = 4) CTAs per SM;  1: <= 256 threads, 3 or 2 CTAs per SM;  2: <= 512 threads
-//   (2 CTAs per SM with P = 2, else 1).
-// The class also fixes the row-buffer pitch (lbc_nfb), hence the shared memory per CTA.
-constexpr int lbc_threads(int lbc) { return lbc == 0 ? 128 : (lbc == 1 ? 256 : 512); }
-// Row-buffer plane pitch in cells, a compile-time constant of the instantiation (so that the 4 S planes sit at immediate
-// offsets): the widest row the class can hold -- nxp <= threads P / 4 data columns -- i.e. (nxp - 1 + NACC) S cells,
-// rounded up to a multiple of 4, plus 4 cells of over-read slack for the vector loads.
-// Bank conflicts.  In the PSF phase neighbouring threads read 16-byte vectors P S elements apart.  When that stride is
-// an EVEN number of vectors (s = 4 with P = 4: 64 B), the 8 lanes of a quarter-warp fall on 2 or 4 of the 8 vector-wide
-// bank groups (ncu, config 5: 7 conflicts per load, L1 pipe 88 % busy).  One pad vector after every P S elements makes
-// the stride odd and the loads conflict-free.  row_pad = pad elements per group of P S (0 when not needed).
-constexpr int row_pad(int P, int S, int elem_bytes) {
-    const int V = 16 / elem_bytes, GRP = P * S;
-    return (GRP % V == 0 && (GRP / V) % 2 == 0) ? V : 0;
-}
-constexpr int lbc_nfb(int lbc, int P, int S, int NACC, int elem_bytes) {
-    const int cells = (lbc_threads(lbc) * P / 4 - 1 + NACC) * S;
-    const int padded = cells + row_pad(P, S, elem_bytes) * ((cells + P * S - 1) / (P * S));
-    return (padded + 3) / 4 * 4 + 4 + row_pad(P, S, elem_bytes);
-}
-constexpr int lbc_blocks(int lbc, int P, bool f64) {
-    return f64 ? (lbc == 0 ? 4 : (lbc == 1 ? 2 : 1))          // fp64 mode: 128 registers in every class
-               : (lbc == 0 ? (P == 2 ? 7 : 6) : (lbc == 1 ? (P == 2 ? 3 : 2) : (P == 2 ? 2 : 1)));
-}
 template <typename T, int S, int NACC, int P, int MODE, int LBC>
 __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T) == 8)) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
@@ -609,7 +726,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
     ThetaC<T>& c = *reinterpret_cast<ThetaC<T>*>(smem_raw);
     constexpr size_t off_tab = (sizeof(ThetaC<T>) + 15) / 16 * 16;
     T* vtab = reinterpret_cast<T*>(smem_raw + off_tab);
-    T* rowbuf = vtab + (size_t)kMaxOct * (1 << TabCfg<T>::M) * NC;
+    T* rowbuf = vtab + ((size_t)kVcOct * (1 << TabCfg<T>::M) + 1) * NC;
     constexpr int nfb = lbc_nfb(LBC, P, S, NACC, (int)sizeof(T));
     constexpr int GRP = P * S, PADV = row_pad(P, S, (int)sizeof(T));
     double* red = reinterpret_cast<double*>(rowbuf + (size_t)S * 4 * nfb);
@@ -624,20 +741,25 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
     const int nsuper = g.ny + NACC - 1;
     const size_t npix = (size_t)g.nx * g.ny;
     const T* run_base = rowbuf + (size_t)q * nfb + grp * (GRP + PADV);
+    const T* bbase = p.btab.coef - (ptrdiff_t)p.btab.first * (2 * NC);
 
     for (int i = tid; i < S * 4 * nfb; i += NT) rowbuf[i] = T(0);
 
     for (int b = blockIdx.x; b < p.B; b += gridDim.x) {
         __syncthreads();
-        if (tid == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, c);
+        if (tid == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.Ftab, c);
         __syncthreads();
-        if (!c.valid) {                              // out-of-domain theta: NaN maps / -inf likelihood
+        if (!c.valid || (c.slow && !p.slow_list)) {  // out-of-domain theta: NaN maps / -inf likelihood
             if constexpr (MODE == 0) {
                 const T qnan = (T)nan("");
                 for (size_t i = tid; i < 4 * npix; i += NT) p.maps[(size_t)b * 4 * npix + i] = qnan;
             } else if (tid == 0) {
                 p.logL[b] = -INFINITY;
             }
+            continue;
+        }
+        if (c.slow) {                                // radii outside the tabulated ranges: left to k_slow (direct path)
+            if (tid == 0) p.slow_list[atomicAdd(p.slow_count, 1)] = b;
             continue;
         }
         build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
@@ -655,8 +777,8 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
             // the per-theta constants are re-read from shared memory for every super-row (a handful of broadcast loads)
             // so that they do not occupy registers during the PSF phase
             const CellK<T> k = load_cellk<T>(c);
-            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, GRP, PADV, false>(g.comps, k, p.btab, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
-            else eval_superrow_any<T, S, nfb, GRP, PADV, true>(g.comps, k, p.btab, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, GRP, PADV, false>(g.comps, k, bbase, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            else eval_superrow_any<T, S, nfb, GRP, PADV, true>(g.comps, k, bbase, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
             vt = vt + 32 < NT ? vt + 32 : vt + 32 - NT;      // rotate the column ownership by one warp: the ragged last
                                                              // pass then falls on a different warp (scheduler) each time
             __syncthreads();
@@ -697,8 +819,8 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
                             if (px < g.nx) p.maps[((size_t)b * 4 + q) * npix + (size_t)py * g.nx + px] = m;
                         } else {
                             const double z = (de[i].x - (double)m) * de[i].y;      // eq. 18, residual in fp64
-                            chi2 = fma(z, z, chi2);                                // padded pixels: 1/e = 0, m finite
-                        }
+                            chi2 = de[i].y != 0.0 ? fma(z, z, chi2) : chi2;        // masked or padded pixel (1/e = 0): the
+                        }                                                          // model value never enters (reading M)
                     }
                 }
 #pragma unroll
@@ -730,6 +852,7 @@ struct FineParams {
     GridC g;
     FitC fit;
     PolyTab<T> btab, Ftab;
+    DirectC direct;
     const double* theta;
     int B;
     T* fine;                     // [B][4][nfy][nfx]
@@ -742,12 +865,12 @@ __global__ void __launch_bounds__(256) k_fine(const __grid_constant__ FineParams
     ThetaC<T>& c = *reinterpret_cast<ThetaC<T>*>(smem_raw);
     constexpr size_t off_tab = (sizeof(ThetaC<T>) + 15) / 16 * 16;
     T* vtab = reinterpret_cast<T*>(smem_raw + off_tab);
-    (void)NC;
     const GridC& g = p.g;
     const size_t plane = (size_t)g.nfx * g.nfy;
+    const T* bbase = p.btab.coef - (ptrdiff_t)p.btab.first * (2 * NC);
     for (int b = blockIdx.x; b < p.B; b += gridDim.x) {
         __syncthreads();
-        if (threadIdx.x == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, c);
+        if (threadIdx.x == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.Ftab, c);
         __syncthreads();
         T* out = p.fine + (size_t)b * 4 * plane;
         if (!c.valid) {
@@ -755,9 +878,14 @@ __global__ void __launch_bounds__(256) k_fine(const __grid_constant__ FineParams
             for (size_t i = threadIdx.x; i < 4 * plane; i += blockDim.x) out[i] = qnan;
             continue;
         }
-        build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
         const CellK<T> k = load_cellk<T>(c);
-        eval_rows_any<T>(g.comps, g.flux != 0, k, p.btab, vtab, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy,
+        if (c.slow) {
+            eval_rows_direct<T>(g.flux != 0, c, g, p.btab, p.Ftab, p.direct, k, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy,
+                                threadIdx.x, blockDim.x);
+            continue;
+        }
+        build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
+        eval_rows_any<T>(g.comps, g.flux != 0, k, bbase, vtab, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy,
                          make_walk(threadIdx.x, blockDim.x, g.nfx), blockDim.x);
     }
 }

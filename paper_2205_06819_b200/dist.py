@@ -67,3 +67,18 @@ def gather_logl(local, B: int, rank: int, world: int):
     out = [torch.empty_like(buf) for _ in range(world)]
     dist.all_gather(out, buf)
     return torch.cat([o[:n] for o, n in zip(out, sizes)])
+
+
+def loglike_sharded(ctx, theta, rank: int | None = None, world: int | None = None):
+    """SURVEY.md sec. 8(e) as one call: theta[B][17] (the same full batch on every rank) -> logL[B] on every rank.
+    Each rank evaluates its contiguous shard with `ctx.loglike` (any object with that method: a bang.Context bound
+    to the rank's GPU) and the shards are all-gathered in batch order.  No collective touches the data path."""
+    import torch
+    import torch.distributed as dist
+    if rank is None or world is None:
+        on = dist.is_available() and dist.is_initialized()
+        rank, world = (dist.get_rank(), dist.get_world_size()) if on else (0, 1)
+    B = theta.shape[0]
+    lo, hi = shard_bounds(B, rank, world)
+    local = ctx.loglike(theta[lo:hi]) if hi > lo else torch.empty(0, dtype=torch.float64, device=getattr(ctx, "device", "cpu"))
+    return gather_logl(local, B, rank, world)

@@ -33,6 +33,15 @@ def _worker(rank, world, port, B, q):
     # stand-in for the per-rank likelihood: any function of the rank's own theta rows (the real one needs a GPU)
     local = torch.as_tensor(mine.sum(axis=1))
     full = D.gather_logl(local, B, rank, world)
+
+    class StubContext:                       # the same stand-in behind bang.Context's loglike(theta) -> logL interface
+        device = "cpu"
+
+        def loglike(self, th):
+            return torch.as_tensor(np.asarray(th).sum(axis=1))
+
+    sharded = D.loglike_sharded(StubContext(), theta)          # the sec. 8(e) entry point: shard -> evaluate -> all-gather
+    assert torch.equal(sharded, full)
     t = D.max_over_ranks(1.0 + rank)
     n = D.sum_over_ranks(float(len(mine)))
     q.put((rank, full.numpy(), t, n))

@@ -94,7 +94,8 @@ def test_empty_batch_is_a_noop(bang, oracle):
     assert ctx.loglike_host(np.zeros((0, 17))).shape == (0,)
     n = ctx.launches
     ctx.loglike(THETA)
-    assert ctx.launches == n + 1                                  # one fused kernel per batch
+    assert ctx.launches == n + 2                                  # one fused kernel per batch + the (empty) direct-path
+                                                                  # launch for theta outside the tabulated ranges
     ctx.close()
 
 
