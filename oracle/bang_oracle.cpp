@@ -325,6 +325,16 @@ Theta decode(const double *th, unsigned comps) {
     return t;
 }
 
+// circular speed squared of everything but the bulge at radius x (eq. 9 per disc, halo): the "external" potential of
+// reading U'
+double vc2_ext(double x, const Theta &t, unsigned comps, int halo_profile) {
+    double v2 = 0.0;
+    for (int j = 0; j < 2; ++j)
+        if (comps & (j ? C_DISC2 : C_DISC1)) v2 += vc2_expdisc(x, t.Md[j], t.Rd[j]);
+    if (comps & C_HALO) v2 += (halo_profile == 1) ? vc2_nfw(x, t.Mh, t.Rh) : vc2_hernquist(x, t.Mh, t.Rh);
+    return v2;
+}
+
 struct Setup {
     int nx, ny, s, rk, nfx, nfy, NJ;
     double pix, kappa;
@@ -332,6 +342,8 @@ struct Setup {
     int halo_profile;                  // 0 Hernquist (paper), 1 NFW (reading H)
     int bulge_profile;                 // 0 Hernquist (paper default), 1 Jaffe (App. B)
     int psf_weighting;                 // 0: the paper's eq. 21 on B, v, sigma, <L/M> (reading G); 1: flux-weighted moments (reading G')
+    int bulge_potential;               // 0: the bulge's dispersion in its own potential (the paper); 1: in the
+                                       //    total potential of eq. 10 (reading U')
     std::vector<double> taps, glx, glw;
 };
 
@@ -352,22 +364,50 @@ void psf_taps(double sigma_pix, int s, double trunc, std::vector<double> &g) {
     for (double &v : g) v /= sum;
 }
 
-// profiles: bits 0-7 halo profile, bits 8-15 bulge profile, bits 16-23 PSF weighting
+// profiles: bits 0-7 halo profile, bits 8-15 bulge profile, bits 16-23 PSF weighting, bits 24-31 bulge potential
 bool make_setup(Setup &S, int nx, int ny, double pix, int s, double dist_mpc, double sigma_pix,
                 double trunc, unsigned comps, int profiles, int NJ) {
     const int halo_profile = profiles & 0xff, bulge_profile = (profiles >> 8) & 0xff;
-    const int psf_weighting = (profiles >> 16) & 0xff;
-    if (halo_profile > 1 || bulge_profile > 1 || psf_weighting > 1) return false;
+    const int psf_weighting = (profiles >> 16) & 0xff, bulge_potential = (profiles >> 24) & 0xff;
+    if (halo_profile > 1 || bulge_profile > 1 || psf_weighting > 1 || bulge_potential > 1) return false;
     if (nx < 1 || ny < 1 || s < 1 || !(pix > 0) || !(dist_mpc > 0) || sigma_pix < 0 || NJ < 1) return false;
     if (!(comps & (C_BULGE | C_DISC1 | C_DISC2))) return false;
     S.nx = nx; S.ny = ny; S.s = s; S.pix = pix; S.kappa = dist_mpc * kArcsecKpcPerMpc;
-    S.comps = comps; S.halo_profile = halo_profile; S.bulge_profile = bulge_profile; S.psf_weighting = psf_weighting; S.NJ = NJ;
+    S.comps = comps; S.halo_profile = halo_profile; S.bulge_profile = bulge_profile; S.psf_weighting = psf_weighting; S.bulge_potential = bulge_potential; S.NJ = NJ;
     psf_taps(sigma_pix, s, trunc, S.taps);
     S.rk = (int(S.taps.size()) - 1) / 2;
     S.nfx = nx * s + 2 * S.rk; S.nfy = ny * s + 2 * S.rk;
     S.glx.resize(NJ); S.glw.resize(NJ);
     gauss_legendre(NJ, S.glx.data(), S.glw.data());
     return true;
+}
+
+// ---- reading U' (variant; PAPER.md:107 and :417-419 name it as the model's first limitation): the bulge's dispersion in
+// the TOTAL potential.  Isotropic spherical Jeans equation with the enclosed mass read off the total circular speed of
+// eq. 10, G M(<x) = x v_c,tot^2(x):   rho_b v_r^2 (r) = int_r^inf rho_b(x) v_c,tot^2(x) / x dx,
+// and its l.o.s. integral with the order of integration exchanged (z <= sqrt(x^2 - R^2)), an exact identity:
+//     I_b(R) = Sigma_b sigma_b^2 = 2 int_0^inf rho_b v_r^2 (sqrt(R^2+z^2)) dz = 2 int_R^inf rho_b(x) v_c,tot^2(x) sqrt(x^2 - R^2) / x dx.
+// v_c,tot^2 = v_c,b^2 + v_ext^2: the bulge's own part is eq. 6 exactly as in the paper's path (Ib_quadrature above), so
+// the variant reduces to it identically when discs and halo vanish; the part of the other components is
+//     I_ext(R) = 2 int_R^inf rho_b(x) v_ext^2(x) sqrt(x^2 - R^2) / x dx,   v_ext^2 = sum_j eq. 9 + halo,
+// by the N_J-node Gauss-Legendre rule on t in (0,1) with x = R + L t^2/(1-t), L = sqrt(R^2 + R_b^2) (the map of reading B:
+// sqrt(x^2 - R^2) = t sqrt(L (2R + d)/(1-t)), d = x - R, is smooth in t).  rho_b: eq. 1 (Hernquist) or eq. B1 (Jaffe).
+double rho_bulge(double x, double Mb, double Rb, int bulge_profile) {
+    if (bulge_profile == 1) return Mb * Rb / (4 * kPi * x * x * (x + Rb) * (x + Rb));        // eq. B1
+    return Mb * Rb / (2 * kPi * x * (x + Rb) * (x + Rb) * (x + Rb));                          // eq. 1
+}
+double Ib_ext_quadrature(double R, const Theta &t, unsigned comps, int halo_profile, int bulge_profile, double Mb, double Rb,
+                         int NJ, const double *glx, const double *glw) {
+    double L = std::sqrt(R * R + Rb * Rb), sum = 0.0;
+    for (int k = 0; k < NJ; ++k) {
+        double tt = 0.5 * (glx[k] + 1.0), wt = 0.5 * glw[k];
+        double d = L * tt * tt / (1.0 - tt);                      // x - R
+        double dxdt = L * tt * (2.0 - tt) / ((1.0 - tt) * (1.0 - tt));
+        double x = R + d;
+        double root = std::sqrt(d * (2.0 * R + d));               // sqrt(x^2 - R^2) without cancellation
+        sum += wt * dxdt * rho_bulge(x, Mb, Rb, bulge_profile) * vc2_ext(x, t, comps, halo_profile) * root / x;
+    }
+    return 2.0 * sum;
 }
 
 // ---- one fine cell: steps 1-8 of the definition (PAPER.md secs 2.1-2.4) -------------
@@ -396,6 +436,8 @@ void fine_cell(const Setup &S, const Theta &t, int Jx, int Jy, double out[4]) {
         Ib = Ib_quadrature_jaffe(R, t.Mb, t.Rb, S.NJ, S.glx.data(), S.glw.data());
         vc2 += vc2_jaffe(r, t.Mb, t.Rb);
     }
+    if ((S.comps & C_BULGE) && S.bulge_potential == 1)          // reading U': + the discs' and the halo's pull on the bulge
+        Ib += Ib_ext_quadrature(R, t, S.comps, S.halo_profile, S.bulge_profile, t.Mb, t.Rb, S.NJ, S.glx.data(), S.glw.data());
     // 5. discs: eq. 7-8;  6. circular speed: eq. 2, 9, 10
     double Sd[2] = {0.0, 0.0};
     for (int j = 0; j < 2; ++j)
@@ -542,6 +584,16 @@ double bo_Ib_quadrature_jaffe(double R, double Mb, double Rb, int NJ) {
     gauss_legendre(NJ, x.data(), w.data());
     return Ib_quadrature_jaffe(R, Mb, Rb, NJ, x.data(), w.data());
 }
+// reading U': I_ext(R) for a bulge (Mb, Rb, profile) in the field of up to two discs and a halo (pins)
+double bo_Ib_ext_quadrature(double R, double Mb, double Rb, int bulge_profile, double Md1, double Rd1, double Md2, double Rd2,
+                            double Mh, double Rh, int halo_profile, unsigned comps, int NJ) {
+    Theta t{};
+    t.Mb = Mb; t.Rb = Rb; t.Md[0] = Md1; t.Rd[0] = Rd1; t.Md[1] = Md2; t.Rd[1] = Rd2; t.Mh = Mh; t.Rh = Rh;
+    std::vector<double> x(NJ), w(NJ);
+    gauss_legendre(NJ, x.data(), w.data());
+    return Ib_ext_quadrature(R, t, comps, halo_profile, bulge_profile, Mb, Rb, NJ, x.data(), w.data());
+}
+double bo_rho_bulge(double x, double Mb, double Rb, int bulge_profile) { return rho_bulge(x, Mb, Rb, bulge_profile); }
 double bo_G() { return kG; }
 double bo_kappa(double dist_mpc) { return dist_mpc * kArcsecKpcPerMpc; }
 

@@ -49,6 +49,8 @@ def lib():
             "bo_jaffe_sigma_tilde": [_d], "bo_jaffe_I_tilde_closed": [_d], "bo_J3": [_d],
             "bo_rho_vr2_jaffe": [_d, _d, _d], "bo_vr2_jaffe_corrected": [_d, _d, _d], "bo_vc2_jaffe": [_d, _d, _d],
             "bo_Ib_quadrature_jaffe": [_d, _d, _d, _i],
+            "bo_Ib_ext_quadrature": [_d, _d, _d, _i, _d, _d, _d, _d, _d, _d, _i, _u, _i],
+            "bo_rho_bulge": [_d, _d, _d, _i],
         }.items():
             f = getattr(L, name)
             f.argtypes, f.restype = args, _d
@@ -80,10 +82,12 @@ def get_threads() -> int:
 
 def _cfg(cfg):
     """cfg: dict with nx ny pix_arcsec supersample dist_mpc sigma_pix trunc_nsigma components halo_profile
-    [bulge_profile] jeans_nodes.  The switches travel in one int: halo | bulge << 8 | psf_weighting << 16."""
+    [bulge_profile] jeans_nodes.  The switches travel in one int: halo | bulge << 8 | psf_weighting << 16 |
+    bulge_potential << 24."""
     return (int(cfg["nx"]), int(cfg["ny"]), float(cfg["pix_arcsec"]), int(cfg["supersample"]),
             float(cfg["dist_mpc"]), float(cfg["sigma_pix"]), float(cfg.get("trunc_nsigma", 3.0)),
-            int(cfg["components"]), int(cfg.get("halo_profile", 0)) | (int(cfg.get("bulge_profile", 0)) << 8) | (int(cfg.get("psf_weighting", 0)) << 16),
+            int(cfg["components"]), int(cfg.get("halo_profile", 0)) | (int(cfg.get("bulge_profile", 0)) << 8) | (int(cfg.get("psf_weighting", 0)) << 16)
+            | (int(cfg.get("bulge_potential", 0)) << 24),
             int(cfg["jeans_nodes"]))
 
 

@@ -606,9 +606,15 @@ constexpr int lbc_nfb(int lbc, int P, int S, int NACC, int elem_bytes) {
     const int padded = cells + row_pad(P, S, elem_bytes) * ((cells + P * S - 1) / (P * S));
     return (padded + 3) / 4 * 4 + 4 + row_pad(P, S, elem_bytes);
 }
+#ifndef BANG_MB_P4
+#define BANG_MB_P4 6             // resident CTAs per SM the class-0 kernels are compiled for (register budget 80 / 72)
+#endif
+#ifndef BANG_MB_P2
+#define BANG_MB_P2 7
+#endif
 constexpr int lbc_blocks(int lbc, int P, bool f64) {
     return f64 ? (lbc == 0 ? 4 : (lbc == 1 ? 2 : 1))          // fp64 mode: 128 registers in every class
-               : (lbc == 0 ? (P == 2 ? 7 : 6) : (lbc == 1 ? (P == 2 ? 3 : 2) : (P == 2 ? 2 : 1)));
+               : (lbc == 0 ? (P == 2 ? BANG_MB_P2 : BANG_MB_P4) : (lbc == 1 ? (P == 2 ? 3 : 2) : (P == 2 ? 2 : 1)));
 }
 
 // a2 + a3 for one super-row of the fused kernel (S fine rows jy0 .. jy0+S-1 = one data row): thread `vt` takes the fine
