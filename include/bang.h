@@ -65,6 +65,11 @@ extern "C" {
                                     and to the mass surface density; v = M1/M0, sigma^2 = M2/M0 - v^2, M/L = M3/M0.
                                     bang_model_fine then returns those four moment fields.  A side variant, run UNFUSED
                                     (moment fields through HBM scratch, several kernels per call), not the tuned path */
+#define BANG_POTENTIAL_SELF  0    /* the paper: the bulge's dispersion in its own potential, eq. 6 */
+#define BANG_POTENTIAL_TOTAL 1    /* variant (reading U'; PAPER.md:417-419 names the approximation above as the model's first
+                                    limitation): Sigma_b sigma_b^2 gains I_ext(R) = 2 int_R^inf rho_b v_ext^2 sqrt(x^2-R^2)/x dx,
+                                    v_ext^2 = discs (eq. 9) + halo, by the same N_J-node rule -- the isotropic Jeans
+                                    equation in the total potential of eq. 10.  Tabulated per theta inside the fused kernel */
 #define BANG_FP32 0              /* fp32 model arithmetic; residuals and logL accumulation in fp64 */
 #define BANG_FP64 1              /* everything in fp64 */
 
@@ -89,6 +94,7 @@ typedef struct {
     int jeans_nodes;       /* N_J >= 1: nodes of the Gauss-Legendre rule for the bulge Jeans l.o.s. integral (reading B) */
     int precision;         /* BANG_FP32 or BANG_FP64 */
     int psf_weighting;     /* BANG_PSF_FIELDS (the paper) or BANG_PSF_FLUX */
+    int bulge_potential;   /* BANG_POTENTIAL_SELF (the paper) or BANG_POTENTIAL_TOTAL */
 } bang_model;
 
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (NULL = the legacy default stream) on

@@ -19,6 +19,8 @@ HALO_HERNQUIST, HALO_NFW = 0, 1
 BULGE_HERNQUIST, BULGE_JAFFE = 0, 1
 FP32, FP64 = 0, 1
 PSF_FIELDS, PSF_FLUX = 0, 1
+POTENTIAL_SELF, POTENTIAL_TOTAL = 0, 1
+HAS_TOTAL_POTENTIAL = True        # bench.py's sweep row for reading U'
 NTHETA = 17
 OK, EINVAL, ENOMEM, ECUDA, ENODATA = 0, -1, -2, -3, -4
 
@@ -38,7 +40,7 @@ class Psf(C.Structure):
 
 class Model(C.Structure):
     _fields_ = [("components", C.c_uint), ("bulge_profile", C.c_int), ("halo_profile", C.c_int),
-                ("jeans_nodes", C.c_int), ("precision", C.c_int), ("psf_weighting", C.c_int)]
+                ("jeans_nodes", C.c_int), ("precision", C.c_int), ("psf_weighting", C.c_int), ("bulge_potential", C.c_int)]
 
 
 class BangError(RuntimeError):
@@ -103,7 +105,7 @@ class Context:
         g = Grid(self.nx, self.ny, float(cfg["pix_arcsec"]), self.s, float(cfg["dist_mpc"]))
         p = Psf(float(cfg["sigma_pix"]), float(cfg.get("trunc_nsigma", 3.0)))
         m = Model(int(cfg["components"]), int(cfg.get("bulge_profile", 0)), int(cfg.get("halo_profile", 0)), int(cfg["jeans_nodes"]),
-                  FP64 if prec == "fp64" else FP32, int(cfg.get("psf_weighting", 0)))
+                  FP64 if prec == "fp64" else FP32, int(cfg.get("psf_weighting", 0)), int(cfg.get("bulge_potential", 0)))
         self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         h = C.c_void_p()
         rc = lib().bang_create(C.byref(h), C.byref(g), C.byref(p), C.byref(m), device,

@@ -30,6 +30,7 @@ struct bang_ctx {
     double2* data = nullptr; double C0 = 0.0; bool has_data = false;
     double* scal = nullptr;                // device scratch: {C0, bad-pixel count}
     double* gl_dev = nullptr;              // N_J Gauss-Legendre nodes then weights (reading B): table build, direct path
+    double2* qd_dev = nullptr; float2* qf_dev = nullptr;   // the same rule as {a_k, b_k} pairs (reading U', ext_Itilde)
     // staging for the *_host calls
     double* h_theta = nullptr; double* d_theta = nullptr; void* h_out = nullptr; void* d_out = nullptr;
     size_t cap_theta = 0, cap_out = 0;
@@ -282,11 +283,17 @@ cudaError_t dispatch_fused(const bang_ctx* c, const FusedLaunch& L, FusedInfo* i
     }
 }
 
+QuadC make_quad(const bang_ctx* c) { return QuadC{c->qd_dev, c->qf_dev, c->model.jeans_nodes}; }
+DirectC make_direct(const bang_ctx* c) {
+    return DirectC{c->gl_dev, c->gl_dev + c->model.jeans_nodes, c->model.jeans_nodes, make_quad(c)};
+}
+
 FusedLaunch make_launch(bang_ctx* c, const double* theta, int B, int mode, void* maps, double* logL) {
     FusedLaunch L{};
     L.g = c->g; L.fit = c->fit;
     L.btab = c->btab; L.btab_first = c->btab_first; L.btab_cells = c->btab_cells;
     L.Ftab = c->Ftab; L.Ftab_first = c->Ftab_first; L.Ftab_cells = c->Ftab_cells;
+    L.quad = make_quad(c);
     L.W = c->W.data(); L.nacc = c->nacc;
     L.theta = theta; L.B = B; L.P = c->P; L.nxp = c->nxp; L.mode = mode;
     L.maps = maps; L.data = c->data; L.C0 = c->C0; L.logL = logL;
@@ -317,7 +324,7 @@ int run_slow(bang_ctx* ctx, const double* theta_dev, int mode, void* maps_dev, d
     p.g = ctx->g;
     p.btab = PolyTab<T>{static_cast<const T*>(ctx->btab), ctx->btab_first, ctx->btab_cells};
     p.Ftab = PolyTab<T>{static_cast<const T*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells};
-    p.direct = DirectC{ctx->gl_dev, ctx->gl_dev + ctx->model.jeans_nodes, ctx->model.jeans_nodes};
+    p.direct = make_direct(ctx);
     p.W = ctx->W_dev; p.nacc = ctx->nacc;
     p.theta = theta_dev; p.slow_list = ctx->slow_list; p.slow_count = ctx->slow_cnt; p.done = ctx->slow_cnt + 1;
     p.maps = static_cast<T*>(maps_dev); p.data = ctx->data; p.P = ctx->P; p.gmax = data_gmax(ctx);
@@ -379,17 +386,17 @@ int run_flux(bang_ctx* ctx, const double* theta_dev, int B, int mode, void* maps
         CU(cudaMalloc(&ctx->fx_chi2, (size_t)B * g.ny * sizeof(double)));
         ctx->fx_chi2_cap = (size_t)B * g.ny;
     }
-    const size_t smem = fused_smem_bytes<T>(0, 0);
+    const size_t smem = fused_smem_bytes<T>(g, 0, 0);
     CU(cudaFuncSetAttribute(k_fine<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int gmax = data_gmax(ctx);
-    const DirectC direct{ctx->gl_dev, ctx->gl_dev + ctx->model.jeans_nodes, ctx->model.jeans_nodes};
+    const DirectC direct = make_direct(ctx);
     for (int b0 = 0; b0 < B; b0 += ctx->fx_chunk) {
         const int Bc = std::min(ctx->fx_chunk, B - b0);
         const double* th = theta_dev + (size_t)b0 * kNTheta;
         const PolyTab<T> Ft{static_cast<const T*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells};
-        k_theta_valid<T><<<(Bc + 127) / 128, 128, 0, ctx->stream>>>(th, Bc, g, Ft, ctx->fx_valid);
-        FineParams<T> fp{g, ctx->fit, PolyTab<T>{static_cast<const T*>(ctx->btab), ctx->btab_first, ctx->btab_cells},
-                         Ft, direct, th, Bc, static_cast<T*>(ctx->fx_fine)};
+        const PolyTab<T> Bt{static_cast<const T*>(ctx->btab), ctx->btab_first, ctx->btab_cells};
+        k_theta_valid<T><<<(Bc + 127) / 128, 128, 0, ctx->stream>>>(th, Bc, g, Bt, Ft, ctx->fx_valid);
+        FineParams<T> fp{g, ctx->fit, Bt, Ft, direct, (int)bs_elems<T>(g), th, Bc, static_cast<T*>(ctx->fx_fine)};
         k_fine<T><<<std::min(Bc, 8 * ctx->n_sm), 256, smem, ctx->stream>>>(fp);
         MomentsParams<T> mp{g, ntap, ctx->W_dev, static_cast<const T*>(ctx->fx_fine), Bc, b0, ctx->fx_valid,
                             static_cast<T*>(maps_dev), ctx->data, ctx->P, gmax, ctx->fx_chi2, mode};
@@ -484,7 +491,7 @@ void bang_destroy(bang_ctx* ctx) {
     if (!ctx) return;
     DeviceGuard dg(ctx->device);
     cudaStreamSynchronize(ctx->stream);
-    cudaFree(ctx->btab); cudaFree(ctx->Ftab); cudaFree(ctx->data); cudaFree(ctx->scal); cudaFree(ctx->gl_dev);
+    cudaFree(ctx->btab); cudaFree(ctx->Ftab); cudaFree(ctx->data); cudaFree(ctx->scal); cudaFree(ctx->gl_dev); cudaFree(ctx->qd_dev); cudaFree(ctx->qf_dev);
     cudaFree(ctx->d_theta); cudaFree(ctx->d_out);
     cudaFree(ctx->slow_list); cudaFree(ctx->slow_cnt);
     cudaFree(ctx->W_dev); cudaFree(ctx->fx_fine); cudaFree(ctx->fx_valid); cudaFree(ctx->fx_chi2);
@@ -509,6 +516,7 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     if (model->jeans_nodes < 1 || model->jeans_nodes > 4096) return BANG_EINVAL;
     if (model->precision != BANG_FP32 && model->precision != BANG_FP64) return BANG_EINVAL;
     if (model->psf_weighting != BANG_PSF_FIELDS && model->psf_weighting != BANG_PSF_FLUX) return BANG_EINVAL;
+    if (model->bulge_potential != BANG_POTENTIAL_SELF && model->bulge_potential != BANG_POTENTIAL_TOTAL) return BANG_EINVAL;
 
     const int s = grid->supersample;
     const int rk = (int)std::ceil(psf->trunc_nsigma * psf->sigma_pix * s - 1e-9);
@@ -538,6 +546,7 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     g.h = grid->pix_arcsec * grid->dist_mpc * kKpcPerArcsecPerMpc / s;
     g.comps = model->components; g.halo_profile = model->halo_profile; g.bulge_profile = model->bulge_profile;
     g.flux = model->psf_weighting;
+    g.bulge_potential = model->bulge_potential;
 
     // eq. 21 on the fine grid, separable (reading F): g[m] = exp(-m^2/(2 sigma_f^2)), normalised;
     // composed with the s-cell box of the rebin: W[t] = (1/s) sum_{b<s} g[t - b], t = 0 .. 2 r_k + s - 1.
@@ -584,6 +593,22 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
         if (cudaMalloc(&ctx->gl_dev, gl.size() * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
         if (cudaMemcpyAsync(ctx->gl_dev, gl.data(), gl.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess) {
             rc = BANG_ECUDA; break;
+        }
+        {   // the rule in the form ext_Itilde takes (reading U'): a_k = t^2/(1-t), b_k = w t (2-t)/(1-t)^2 on t in (0,1)
+            const int NJ = model->jeans_nodes;
+            std::vector<double2> qd(NJ);
+            std::vector<float2> qf(NJ);
+            for (int k = 0; k < NJ; ++k) {
+                const long double t = 0.5L * ((long double)gl[k] + 1.0L), w = 0.5L * (long double)gl[NJ + k];
+                const long double a = t * t / (1.0L - t), b = w * t * (2.0L - t) / ((1.0L - t) * (1.0L - t));
+                qd[k] = make_double2((double)a, (double)b);
+                qf[k] = make_float2((float)a, (float)b);
+            }
+            if (cudaMalloc(&ctx->qd_dev, NJ * sizeof(double2)) != cudaSuccess || cudaMalloc(&ctx->qf_dev, NJ * sizeof(float2)) != cudaSuccess) {
+                rc = BANG_ENOMEM; break;
+            }
+            if (cudaMemcpy(ctx->qd_dev, qd.data(), NJ * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess ||
+                cudaMemcpy(ctx->qf_dev, qf.data(), NJ * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) { rc = BANG_ECUDA; break; }
         }
         rc = f64 ? build_universal<double>(ctx, ctx->gl_dev, ctx->gl_dev + model->jeans_nodes)
                  : build_universal<float>(ctx, ctx->gl_dev, ctx->gl_dev + model->jeans_nodes);
@@ -672,21 +697,21 @@ int bang_model_fine(bang_ctx* ctx, const double* theta_dev, int B, void* fine_de
     ON_DEVICE(ctx);
     const bool f64 = ctx->model.precision == BANG_FP64;
     const int ctas = std::min(B, 8 * ctx->n_sm);
-    const DirectC direct{ctx->gl_dev, ctx->gl_dev + ctx->model.jeans_nodes, ctx->model.jeans_nodes};
+    const DirectC direct = make_direct(ctx);
     if (f64) {
         FineParams<double> p{ctx->g, ctx->fit,
                              PolyTab<double>{static_cast<const double*>(ctx->btab), ctx->btab_first, ctx->btab_cells},
                              PolyTab<double>{static_cast<const double*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells},
-                             direct, theta_dev, B, static_cast<double*>(fine_dev)};
-        const size_t smem = fused_smem_bytes<double>(0, 0);
+                             direct, (int)bs_elems<double>(ctx->g), theta_dev, B, static_cast<double*>(fine_dev)};
+        const size_t smem = fused_smem_bytes<double>(ctx->g, 0, 0);
         CU(cudaFuncSetAttribute(k_fine<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_fine<double><<<ctas, 256, smem, ctx->stream>>>(p);
     } else {
         FineParams<float> p{ctx->g, ctx->fit,
                             PolyTab<float>{static_cast<const float*>(ctx->btab), ctx->btab_first, ctx->btab_cells},
                             PolyTab<float>{static_cast<const float*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells},
-                            direct, theta_dev, B, static_cast<float*>(fine_dev)};
-        const size_t smem = fused_smem_bytes<float>(0, 0);
+                            direct, (int)bs_elems<float>(ctx->g), theta_dev, B, static_cast<float*>(fine_dev)};
+        const size_t smem = fused_smem_bytes<float>(ctx->g, 0, 0);
         CU(cudaFuncSetAttribute(k_fine<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_fine<float><<<ctas, 256, smem, ctx->stream>>>(p);
     }

@@ -17,7 +17,7 @@ template <typename T, int S, int NACC, int P, int MODE, int LBC>
 cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) {
     auto kern = k_fused<T, S, NACC, P, MODE, LBC>;
     if (L.threads > lbc_threads(LBC)) return cudaErrorInvalidValue;
-    const size_t smem = fused_smem_bytes<T>(S, lbc_nfb(LBC, P, S, NACC, (int)sizeof(T)));
+    const size_t smem = fused_smem_bytes<T>(L.g, S, lbc_nfb(LBC, P, S, NACC, (int)sizeof(T)));
     // the shared-memory opt-in and the occupancy query are done once per context and mode (L.cache, owned by the
     // context): repeating them on every call costs ~10 us of host time, which a small batch notices
     int per_sm = L.cache ? L.cache[L.mode] : 0;
@@ -51,6 +51,7 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     p.g = L.g; p.fit = L.fit;
     p.btab = PolyTab<T>{static_cast<const T*>(L.btab), L.btab_first, L.btab_cells};
     p.Ftab = PolyTab<T>{static_cast<const T*>(L.Ftab), L.Ftab_first, L.Ftab_cells};
+    p.quad = L.quad; p.bs_elems = (int)bs_elems<T>(L.g);
     for (int t = 0; t < NACC * S; ++t) p.W[t] = (T)L.W[t];
     p.theta = L.theta; p.B = L.B; p.nxp = L.nxp;
     p.maps = static_cast<T*>(L.maps); p.data = L.data; p.C0 = L.C0; p.logL = L.logL;

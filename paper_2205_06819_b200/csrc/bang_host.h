@@ -12,6 +12,7 @@ struct FusedLaunch {
     FitC fit;
     const void* btab; int btab_first, btab_cells;
     const void* Ftab; int Ftab_first, Ftab_cells;
+    QuadC quad;                  // reading U': N_J-node rule as {a_k, b_k} pairs (device)
     const double* W; int nacc;   // composite taps, nacc * s of them
     const double* theta; int B;
     int P, nxp, mode;

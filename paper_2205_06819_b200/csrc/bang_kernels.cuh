@@ -19,6 +19,7 @@ namespace bang {
 
 constexpr int kNTheta = 17;      // Table 1
 constexpr int kVcOct = 32;           // octaves of r^2 the per-theta v_c table holds (a theta that needs more takes the direct path)
+constexpr int kBOct = 24;            // octaves of s^2 = R^2/R_b^2 the per-theta slice of the bulge tables holds (likewise)
 constexpr unsigned C_BULGE = 1u, C_DISC1 = 2u, C_DISC2 = 4u, C_HALO = 8u;
 constexpr int kBulgeOctLo = -44, kBulgeOctHi = 36;    // universal bulge tables: s^2 in [2^-44, 2^36)
 constexpr int kFOctLo = -60, kFOctHi = 10;            // universal Freeman table: y^2 in [2^-60, 2^10)
@@ -55,6 +56,7 @@ struct ThetaD {      // what the table build needs, in double
     double Ad[2], inv2Rd[2];     // disc  v_c^2 = Ad F(r inv2Rd),  Ad = 2 G M_d/R_d  (eq. 9, reading D)
     double Ah, hs;               // halo: Hernquist GMh, Rh;  NFW: G M200/mu(c), 1/r_s  (reading H)
     double ghc, ghs, gxp0, gyp0, gtan2i;   // the geometry of ThetaC (hc, hs, xp0, yp0, tan2i) in double: direct path
+    double s2near;               // s^2 = R^2/R_b^2 of the cell nearest to the centre (entry 0 of the per-theta bulge tables)
 };
 template <typename T>
 struct ThetaC {
@@ -64,6 +66,9 @@ struct ThetaC {
     int vfirst, vcells;          // per-theta v_c table: first global interval, number of regular intervals (entry 0 of the
                                  // table is the constant v_c of the cell nearest to the centre, entries 1.. the intervals)
     T vc_near;                   // v_c at that cell
+    int bfirst, bcells;          // per-theta bulge tables over s^2 = R^2/R_b^2: first global interval, number of regular
+                                 // intervals (entry 0 = the cell nearest to the centre, as for v_c)
+    T sig_near, J_near;          // SigmaTilde and J at that cell
     T hc, hs;                    // h cos PA, h sin PA   (h = fine cell size in kpc)
     T xp0, yp0;                  // rotated offset of cell (jcx, jcy) from the centre
     T tan2i;                     // tan^2 i = 1/cos^2 i - 1
@@ -83,9 +88,14 @@ struct GridC {
     unsigned comps;
     int halo_profile;            // 0 Hernquist (paper), 1 NFW (reading H)
     int bulge_profile;           // 0 Hernquist (paper default), 1 Jaffe (App. B)
-    int flux;                    // 1: flux-weighted PSF variant (reading G'): k_fine writes the light moments; the fused
-                                 // kernel is not used (bang_api.cu runs k_fine + k_psf_moments instead)
+    int flux;                    // 1: flux-weighted PSF variant (reading G'): the fine fields are the light moments
+    int bulge_potential;         // 1: the bulge's dispersion in the total potential (reading U'): + I_ext, see ext_Itilde
 };
+
+// reading U' is active: a bulge, the switch, and something other than the bulge to pull on it
+inline __host__ __device__ bool has_ext(const GridC& g) {
+    return g.bulge_potential && (g.comps & C_BULGE) && (g.comps & (C_DISC1 | C_DISC2 | C_HALO));
+}
 
 struct FitC {                    // Chebyshev-node fit of degree D: nodes t_k and the inverse Vandermonde matrix
     double tnode[8];
@@ -117,20 +127,21 @@ BANG_D double freeman_F_tab(const PolyTab<T>& Ftab, double y2) {
 }
 
 // total circular speed squared at radius r in the disc plane (eq. 10)
+// comps: which terms to sum (g.comps for eq. 10; g.comps & ~C_BULGE for the "external" field of reading U')
 template <typename T>
-BANG_D double vc2_total(const ThetaD& d, const GridC& g, const PolyTab<T>& Ftab, double r) {
+BANG_D double vc2_total(const ThetaD& d, const GridC& g, const unsigned comps, const PolyTab<T>& Ftab, double r) {
     double v2 = 0.0;
-    if (g.comps & C_BULGE) {
+    if (comps & C_BULGE) {
         const double a = r + d.Rb;
         v2 += g.bulge_profile == 1 ? d.GMb / a : d.GMb * r / (a * a);      // eq. B2 / eq. 2
     }
 #pragma unroll
     for (int j = 0; j < 2; ++j)
-        if (g.comps & (j ? C_DISC2 : C_DISC1)) {
+        if (comps & (j ? C_DISC2 : C_DISC1)) {
             const double y = r * d.inv2Rd[j];
             v2 += d.Ad[j] * freeman_F_tab(Ftab, y * y);
         }
-    if (g.comps & C_HALO) {
+    if (comps & C_HALO) {
         if (g.halo_profile == 1) v2 += d.Ah * nfw_mu<double>(r * d.hs) / r;
         else { const double a = r + d.hs; v2 += d.Ah * r / (a * a); }
     }
@@ -160,19 +171,19 @@ BANG_D float freeman_F_tab_f(const PolyTab<float>& Ftab, float y2) {
     return horner<float, TabCfg<float>::D>(Ftab.coef + (size_t)c * (TabCfg<float>::D + 1), t);
 }
 struct ThetaF { float GMb, Rb, Ad[2], inv2Rd[2], Ah, hs; };
-BANG_D float vc2_total_f(const ThetaF& d, const GridC& g, const PolyTab<float>& Ftab, const float r) {
+BANG_D float vc2_total_f(const ThetaF& d, const GridC& g, const unsigned comps, const PolyTab<float>& Ftab, const float r) {
     float v2 = 0.0f;
-    if (g.comps & C_BULGE) {
+    if (comps & C_BULGE) {
         const float ia = 1.0f / (r + d.Rb);
         v2 += g.bulge_profile == 1 ? d.GMb * ia : d.GMb * r * ia * ia;
     }
 #pragma unroll
     for (int j = 0; j < 2; ++j)
-        if (g.comps & (j ? C_DISC2 : C_DISC1)) {
+        if (comps & (j ? C_DISC2 : C_DISC1)) {
             const float y = r * d.inv2Rd[j];
             v2 += d.Ad[j] * freeman_F_tab_f(Ftab, y * y);
         }
-    if (g.comps & C_HALO) {
+    if (comps & C_HALO) {
         if (g.halo_profile == 1) v2 += d.Ah * nfw_mu<float>(r * d.hs) / r;
         else { const float ia = 1.0f / (r + d.hs); v2 += d.Ah * r * ia * ia; }
     }
@@ -181,7 +192,7 @@ BANG_D float vc2_total_f(const ThetaF& d, const GridC& g, const PolyTab<float>& 
 
 // a0: decode theta[17] (Table 1).  Run by ONE thread; everything in fp64.
 template <typename T>
-BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, const PolyTab<T>& Ftab, ThetaC<T>& c) {
+BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, const PolyTab<T>& btab, const PolyTab<T>& Ftab, ThetaC<T>& c) {
     const unsigned comps = g.comps;
     c.valid = 0;
     c.slow = 0;
@@ -232,6 +243,7 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, const Po
     const double lo_m = 1.0 - 0x1p-10, hi_m = 1.0 + 0x1p-10;
     const bool inside = fabs(dx) <= 0.5 * h * hi_m && fabs(dy) <= 0.5 * h * hi_m;
     const double Llo = inside ? fmin(0.25 * h * h, r2max) : R2min;
+    const double LloR = inside ? fmin(0.25 * h * h, R2max) : R2min;           // the same for R^2 (the bulge tables)
     const int e_lo = ilogb(Llo * lo_m), e_hi = ilogb(r2max * hi_m);
     if (e_hi - e_lo + 1 > kVcOct || e_hi > 100) c.slow = 1;                      // direct evaluation (eval_cell_direct)
     // fp32 mode: r^2 = R^2 + y'^2 tan^2 i amplifies the rounding of y' (relative ~2^-23 per operation) by tan i; beyond
@@ -243,13 +255,28 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, const Po
     ThetaD& d = c.d;
     // bulge: eq. 1-6
     c.invRb2 = T(1); c.ampBb = T(0); c.ampIb = T(0); c.MLb = T(1);
-    d.GMb = 0.0; d.Rb = 1.0;
+    c.bfirst = 0; c.bcells = 0; c.sig_near = T(0); c.J_near = T(0);
+    d.GMb = 0.0; d.Rb = 1.0; d.s2near = 1.0;
     if (comps & C_BULGE) {      // eq. 1-6 (Hernquist) or App. B (Jaffe): both scale-free in s = R/R_b
         const double Mb = exp10(th[4]), Rb = th[5], MLb = th[12];
         const double inv = 1.0 / (Rb * Rb);
         // s^2 = R^2/R_b^2 must stay inside the scale-free tables; otherwise the direct path evaluates eq. 4-6 per cell
         if (!(R2min * inv * lo_m >= ldexp(1.0, kBulgeOctLo)) || !(R2max * inv * hi_m < ldexp(1.0, kBulgeOctHi))) c.slow = 1;
         c.invRb2 = (T)inv;
+        // the theta's slice of the scale-free tables: [LloR, R2max] / R_b^2 in regular intervals + entry 0 for the cell
+        // nearest to the centre, exactly as for v_c
+        const int eb_lo = ilogb(LloR * inv * lo_m), eb_hi = ilogb(R2max * inv * hi_m);
+        if (eb_hi - eb_lo + 1 > kBOct) c.slow = 1;
+        c.bfirst = tab_first_cell<T>(eb_lo);
+        c.bcells = c.slow ? 0 : (eb_hi - eb_lo + 1) << TabCfg<T>::M;
+        d.s2near = R2min * inv;
+        if (!c.slow) {
+            T tt;
+            const int cell = min(max(tab_cell((T)d.s2near, tt) - btab.first, 0), btab.n_cells - 1);
+            const T* pc = btab.coef + (size_t)cell * (2 * (TabCfg<T>::D + 1));
+            c.sig_near = horner<T, TabCfg<T>::D>(pc, tt);
+            c.J_near = horner<T, TabCfg<T>::D>(pc + TabCfg<T>::D + 1, tt);
+        }
         if (g.bulge_profile == 1) {
             c.ampBb = (T)(Mb / (Rb * Rb) / MLb * 1e-6);                                  // eq. B4, in Lsun/pc^2
             c.ampIb = (T)(kG * Mb * Mb / (4.0 * kPi * Rb * Rb * Rb) * 2.0 / MLb * 1e-6); // l.o.s. integral of B1 x B3
@@ -289,8 +316,30 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, const Po
         }
     }
     // v_c at the cell nearest to the centre (entry 0 of the per-theta table)
-    c.vc_near = (T)sqrt(vc2_total<T>(d, g, Ftab, sqrt(R2min + yp0 * yp0 * tan2i)));
+    c.vc_near = (T)sqrt(vc2_total<T>(d, g, g.comps, Ftab, sqrt(R2min + yp0 * yp0 * tan2i)));
     c.valid = 1;
+}
+
+// Node values -> monomial coefficients, in place: cells x (D+1) values at the Chebyshev nodes of each interval become the
+// D+1 coefficients of its interpolant (fit.vinv, fp64 arithmetic).  One thread per interval; no barrier inside.
+template <typename T>
+BANG_D void fit_cells(const FitC& fit, T* reg, const int cells) {
+    constexpr int NC = TabCfg<T>::D + 1;
+    for (int cell = threadIdx.x; cell < cells; cell += blockDim.x) {
+        T* p = reg + cell * NC;
+        double f[NC], co[NC];
+#pragma unroll
+        for (int k = 0; k < NC; ++k) f[k] = (double)p[k];
+#pragma unroll
+        for (int d = 0; d < NC; ++d) {
+            double a = 0.0;
+#pragma unroll
+            for (int k = 0; k < NC; ++k) a = fma(fit.vinv[d * NC + k], f[k], a);
+            co[d] = a;
+        }
+#pragma unroll
+        for (int d = 0; d < NC; ++d) p[d] = (T)co[d];
+    }
 }
 
 // a1: the per-theta radial table v_c(r), a piecewise polynomial in u = r^2 on the pseudo-log grid, built cooperatively
@@ -311,7 +360,7 @@ BANG_D void build_vc_table(const ThetaC<T>& c, const GridC& g, const FitC& fit, 
             double lo, width;
             tab_interval<T>(c.vfirst + cell, lo, width);
             const float u = (float)(lo + 0.5 * width * (fit.tnode[k] + 1.0));
-            reg[i] = sqrtf(vc2_total_f(df, g, Ftab, sqrtf(u)));
+            reg[i] = sqrtf(vc2_total_f(df, g, g.comps, Ftab, sqrtf(u)));
         }
     } else {
         for (int i = threadIdx.x; i < n; i += blockDim.x) {
@@ -319,26 +368,135 @@ BANG_D void build_vc_table(const ThetaC<T>& c, const GridC& g, const FitC& fit, 
             double lo, width;
             tab_interval<T>(c.vfirst + cell, lo, width);
             const double u = lo + 0.5 * width * (fit.tnode[k] + 1.0);
-            reg[i] = (T)sqrt(vc2_total(c.d, g, Ftab, sqrt(u)));
+            reg[i] = (T)sqrt(vc2_total(c.d, g, g.comps, Ftab, sqrt(u)));
         }
     }
     __syncthreads();
-    for (int cell = threadIdx.x; cell < c.vcells; cell += blockDim.x) {
-        T* p = reg + cell * NC;
-        double f[NC], co[NC];
-#pragma unroll
-        for (int k = 0; k < NC; ++k) f[k] = (double)p[k];
-#pragma unroll
-        for (int d = 0; d < NC; ++d) {
-            double a = 0.0;
-#pragma unroll
-            for (int k = 0; k < NC; ++k) a = fma(fit.vinv[d * NC + k], f[k], a);
-            co[d] = a;
+    fit_cells<T>(fit, reg, c.vcells);
+    __syncthreads();
+}
+
+// ---- reading U' (variant; PAPER.md:107 and :417-419 name it as the model's first limitation): the bulge's dispersion in
+// the TOTAL potential of eq. 10.  Sigma_b sigma_b^2 gains the pull of the discs and the halo on the bulge's stars,
+//   I_ext(R) = 2 int_R^inf rho_b(x) v_ext^2(x) sqrt(x^2 - R^2)/x dx,   v_ext^2 = sum_j eq. 9 + halo,
+// by the same N_J-node Gauss-Legendre rule as eq. 6 (reading B) on t in (0,1) with x = R + L t^2/(1-t), L = sqrt(R^2+R_b^2).
+// In units of R_b (s = R/R_b, x~ = x/R_b) and of the amplitude ampIb of the scale-free J:
+//   Itilde_ext(s) = I_ext / (2 G M_b^2/(2 pi R_b^3)) [Hernquist; likewise Jaffe] = (R_b/(G M_b)) sum_k L~ b_k rho~(x~_k) v_ext^2(R_b x~_k) root_k/x~_k,
+//   x~_k = s + L~ a_k,  root_k = sqrt(L~ a_k (2 s + L~ a_k)),  a_k = t_k^2/(1-t_k),  b_k = w_k t_k (2-t_k)/(1-t_k)^2 (host, long double),
+//   rho~ = 1/(x~ (1+x~)^3) (eq. 1) or 1/(x~^2 (1+x~)^2) (eq. B1).
+// Unlike J it is not scale-free (it depends on R_d/R_b, R_h/R_b, ...): it is tabulated PER THETA over the s^2 this theta's
+// grid spans -- north_star's kernel (1) in earnest.  R: the arithmetic type (float in fp32 mode, double otherwise).
+struct QuadC {
+    const double2* qd;           // [N_J] {a_k, b_k} (device)
+    const float2* qf;            // the same rounded to fp32
+    int NJ;
+};
+BANG_D void quad_node(const QuadC& q, int k, double& a, double& b) { const double2 v = __ldg(q.qd + k); a = v.x; b = v.y; }
+BANG_D void quad_node(const QuadC& q, int k, float& a, float& b) { const float2 v = __ldg(q.qf + k); a = v.x; b = v.y; }
+template <typename T>
+BANG_D double vext2(const ThetaD& d, const ThetaF&, const GridC& g, const PolyTab<T>& Ftab, double r) {
+    return vc2_total<T>(d, g, g.comps & ~C_BULGE, Ftab, r);
+}
+BANG_D float vext2(const ThetaD&, const ThetaF& df, const GridC& g, const PolyTab<float>& Ftab, float r) {
+    return vc2_total_f(df, g, g.comps & ~C_BULGE, Ftab, r);
+}
+template <typename R, typename T>
+BANG_D R ext_Itilde(const R s, const ThetaD& d, const ThetaF& df, const GridC& g, const PolyTab<T>& Ftab, const QuadC& q) {
+    const R L = sqrt(fma(s, s, R(1)));
+    const R Rb = (R)d.Rb;
+    R sum = R(0);
+#pragma unroll 1
+    for (int k = 0; k < q.NJ; ++k) {
+        R a, b;
+        quad_node(q, k, a, b);
+        const R dd = L * a;                               // x~ - s
+        const R x = s + dd;
+        const R root = sqrt(dd * (R(2) * s + dd));        // sqrt(x~^2 - s^2) without cancellation
+        const R rx = R(1) / x, r1 = R(1) / (R(1) + x);
+        // rho~ root / x~ as a product of reciprocals (no overflow of x~^2 (1+x~)^3 in fp32)
+        const R shape = g.bulge_profile == 1 ? rx * rx * rx * r1 * r1 : rx * rx * r1 * r1 * r1;
+        sum = fma(L * b * root * shape, vext2(d, df, g, Ftab, Rb * x), sum);
+    }
+    return sum * (R)(d.Rb / d.GMb);
+}
+
+// a1 (continued): the per-theta bulge tables in shared memory.
+//   fp32 mode: bs[entry][2][D+1] = {SigmaTilde, J (+ Itilde_ext)} -- entry 0 is the cell nearest to the centre (constants),
+//   entries 1.. are this theta's slice of the scale-free tables, copied from global memory: the per-cell look-up is then
+//   two 128-bit shared loads instead of two gathers through L1.
+//   fp64 mode: the scale-free tables stay in global memory; bs[entry][D+1] = Itilde_ext only, and only for reading U'.
+// scratch: room for (bcells (D+1) + 1) values of T (the row buffer, idle during the prologue).
+// Must be called by all threads; ends with a __syncthreads().
+template <typename T>
+BANG_D void build_bulge_tables(const ThetaC<T>& c, const GridC& g, const FitC& fit, const PolyTab<T>& btab, const PolyTab<T>& Ftab,
+                               const QuadC& q, T* bs, T* scratch) {
+    constexpr int D = TabCfg<T>::D, NC = D + 1;
+    const bool ext = has_ext(g);
+    if constexpr (sizeof(T) == 4) {
+        if (!(g.comps & C_BULGE)) { __syncthreads(); return; }
+        const float4* src = reinterpret_cast<const float4*>(btab.coef + (size_t)(c.bfirst - btab.first) * (2 * NC));
+        float4* dst = reinterpret_cast<float4*>(bs);
+        if (threadIdx.x == 0) {
+            dst[0] = make_float4(c.sig_near, 0.f, 0.f, 0.f);
+            dst[1] = make_float4(c.J_near, 0.f, 0.f, 0.f);
         }
-#pragma unroll
-        for (int d = 0; d < NC; ++d) p[d] = (T)co[d];
+        for (int i = threadIdx.x; i < c.bcells * 2; i += blockDim.x) dst[2 + i] = __ldg(src + i);
+    }
+    if (!ext) { __syncthreads(); return; }
+    // Itilde_ext at the Chebyshev nodes of every interval of the slice (+ the nearest cell), then the fit
+    const int n = c.bcells * NC;
+    if constexpr (sizeof(T) == 4) {
+        const ThetaF df{(float)c.d.GMb, (float)c.d.Rb, {(float)c.d.Ad[0], (float)c.d.Ad[1]},
+                        {(float)c.d.inv2Rd[0], (float)c.d.inv2Rd[1]}, (float)c.d.Ah, (float)c.d.hs};
+        for (int i = threadIdx.x; i <= n; i += blockDim.x) {
+            float s2;
+            if (i == n) s2 = (float)c.d.s2near;
+            else {
+                const int cell = i / NC, k = i - cell * NC;
+                double lo, width;
+                tab_interval<T>(c.bfirst + cell, lo, width);
+                s2 = (float)(lo + 0.5 * width * (fit.tnode[k] + 1.0));
+            }
+            scratch[i] = ext_Itilde<float, float>(sqrtf(s2), c.d, df, g, Ftab, q);
+        }
+    } else {
+        const ThetaF df{};
+        for (int i = threadIdx.x; i <= n; i += blockDim.x) {
+            double s2;
+            if (i == n) s2 = c.d.s2near;
+            else {
+                const int cell = i / NC, k = i - cell * NC;
+                double lo, width;
+                tab_interval<T>(c.bfirst + cell, lo, width);
+                s2 = lo + 0.5 * width * (fit.tnode[k] + 1.0);
+            }
+            scratch[i] = (T)ext_Itilde<double, T>(sqrt(s2), c.d, df, g, Ftab, q);
+        }
     }
     __syncthreads();
+    fit_cells<T>(fit, scratch, c.bcells);
+    __syncthreads();
+    if constexpr (sizeof(T) == 4) {
+        // J += Itilde_ext, coefficient by coefficient (both are polynomials in the same t on the same interval)
+        for (int i = threadIdx.x; i < n; i += blockDim.x) {
+            const int cell = i / NC, k = i - cell * NC;
+            bs[(size_t)(1 + cell) * (2 * NC) + NC + k] += scratch[i];
+        }
+        if (threadIdx.x == 0) bs[NC] += scratch[n];
+    } else {
+        for (int i = threadIdx.x; i < n; i += blockDim.x) bs[NC + i] = scratch[i];
+        if (threadIdx.x < NC) bs[threadIdx.x] = threadIdx.x == 0 ? scratch[n] : T(0);
+    }
+    __syncthreads();
+}
+// number of T values of the per-theta bulge tables (bs above); 0 when the variant does not need them
+template <typename T>
+inline size_t bs_elems(const GridC& g) {
+    constexpr int NC = TabCfg<T>::D + 1;
+    const size_t entries = (size_t)kBOct * (1 << TabCfg<T>::M) + 1;
+    if (!(g.comps & C_BULGE)) return 0;
+    if (sizeof(T) == 4) return entries * 2 * NC;
+    return has_ext(g) ? entries * NC : 0;
 }
 
 // per-theta constants of the fine-cell model, copied from shared memory into registers so that the per-cell code below
@@ -348,6 +506,7 @@ struct CellK {
     int jcx, jcy;
     int vfirst1;                 // global interval number of table entry 0 (= first regular interval - 1)
     int vlast;                   // last valid entry (BANG_CHECK builds only)
+    int bfirst1, blast;          // the same for the per-theta bulge tables
     T hc, hs, xp0, yp0, tan2i;
     T invRb2, ampBb, ampIb, MLb;
     T cexp0, cexp1, ampBd0, ampBd1, ampSd0, ampSd1, vkB0, vkB1, q3B0, q3B1;
@@ -356,6 +515,7 @@ template <typename T>
 BANG_D CellK<T> load_cellk(const ThetaC<T>& c) {
     CellK<T> k;
     k.jcx = c.jcx; k.jcy = c.jcy; k.vfirst1 = c.vfirst - 1; k.vlast = c.vcells;
+    k.bfirst1 = c.bfirst - 1; k.blast = c.bcells;
     k.hc = c.hc; k.hs = c.hs; k.xp0 = c.xp0; k.yp0 = c.yp0; k.tan2i = c.tan2i;
     k.invRb2 = c.invRb2; k.ampBb = c.ampBb; k.ampIb = c.ampIb; k.MLb = c.MLb;
     k.cexp0 = c.cexp[0]; k.cexp1 = c.cexp[1]; k.ampBd0 = c.ampBd[0]; k.ampBd1 = c.ampBd[1];
@@ -397,11 +557,13 @@ BANG_D void combine_cell(const CellK<T>& k, const T Bb, const T IbL, const T E1,
 // a2 + a3: one fine cell at (xp, yp) in the galaxy frame -> B_tot, v_los, sigma_los, <L/M>   (eqs. 4-15, 19).  BULGE: the
 // model has a bulge; SHIFT = 0/1/2/3: without a bulge the disc exponentials are scaled by disc 1 (1), disc 2 (2) or the
 // larger of the two (3) so that the ratios below survive fp32 underflow far outside small discs.
-// bbase: the scale-free bulge table with its first interval folded in (coef - first * 2 (D+1)); the caller guarantees
-// that s^2 and r^2 stay inside the tables (decode_theta: otherwise the theta takes eval_cell_direct).
+// bbase: the scale-free bulge table in global memory with its first interval folded in (coef - first * 2 (D+1)); used in
+// fp64 mode.  bs: the per-theta bulge tables in shared memory (build_bulge_tables): in fp32 mode the theta's slice of
+// {SigmaTilde, J}, in fp64 mode Itilde_ext of reading U' or NULL.  The caller guarantees that s^2 and r^2 stay inside the
+// tables (decode_theta: otherwise the theta takes eval_cell_direct).
 template <typename T, bool BULGE, int SHIFT, bool FLUX = false>
-BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab, const T xp, const T yp,
-                      T& oB, T& oV, T& oS, T& oLM) {
+BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs, const T* __restrict__ vtab,
+                      const T xp, const T yp, T& oB, T& oV, T& oS, T& oLM) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     // (xp, yp): the cell in the galaxy frame; R on the sky (bulge), r in the disc plane
     const T floor2 = sizeof(T) == 4 ? T(0x1p-32f) : T(0x1p-32);
@@ -419,23 +581,40 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bbase, const T* _
     if constexpr (BULGE) {
         T t;
         const int cell = tab_cell(R2 * k.invRb2, t);
-        const T* p = bbase + (ptrdiff_t)cell * (2 * NC);
         T cs[NC], cj[NC];
         if constexpr (sizeof(T) == 4) {
-            const float4 v0 = __ldg(reinterpret_cast<const float4*>(p));
-            const float4 v1 = __ldg(reinterpret_cast<const float4*>(p) + 1);
+            const int e = max(cell - k.bfirst1, 0);                  // entry 0: the cell nearest to the centre
+            BANG_ASSERT(e <= k.blast);
+            const float4* p = reinterpret_cast<const float4*>(bs) + 2 * e;
+            const float4 v0 = p[0], v1 = p[1];
             cs[0] = v0.x; cs[1] = v0.y; cs[2] = v0.z; cs[3] = v0.w;
             cj[0] = v1.x; cj[1] = v1.y; cj[2] = v1.z; cj[3] = v1.w;
+            Bb = k.ampBb * horner<T, D>(cs, t);
+            IbL = k.ampIb * horner<T, D>(cj, t);
         } else {
+            const T* p = bbase + (ptrdiff_t)cell * (2 * NC);
 #pragma unroll
             for (int d = 0; d < NC; d += 2) {
                 const double2 v0 = __ldg(reinterpret_cast<const double2*>(p + d));
                 const double2 v1 = __ldg(reinterpret_cast<const double2*>(p + NC + d));
                 cs[d] = v0.x; cs[d + 1] = v0.y; cj[d] = v1.x; cj[d + 1] = v1.y;
             }
+            Bb = k.ampBb * horner<T, D>(cs, t);
+            T J = horner<T, D>(cj, t);
+            if (bs) {                                                // reading U': + Itilde_ext from the per-theta table
+                const int e = max(cell - k.bfirst1, 0);
+                BANG_ASSERT(e <= k.blast);
+                const T* pe = bs + e * NC;
+                T ce[NC];
+#pragma unroll
+                for (int d = 0; d < NC; d += 2) {
+                    const double2 v0 = *reinterpret_cast<const double2*>(pe + d);
+                    ce[d] = v0.x; ce[d + 1] = v0.y;
+                }
+                J += horner<T, D>(ce, t);
+            }
+            IbL = k.ampIb * J;
         }
-        Bb = k.ampBb * horner<T, D>(cs, t);
-        IbL = k.ampIb * horner<T, D>(cj, t);
     }
     // discs: eq. 7-8
     const T e1a = r * k.cexp0, e2a = r * k.cexp1;
@@ -471,6 +650,7 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bbase, const T* _
 // [2^-22, 2^18): the library's domain is the model's, not the tables'.  ~1e3-1e4 times slower per cell than eval_cell.
 struct DirectC {
     const double* glx; const double* glw; int NJ;   // the Gauss-Legendre rule of reading B (device memory)
+    QuadC quad;                                     // the same rule in the form ext_Itilde takes (reading U')
 };
 template <typename T, bool FLUX>
 __device__ __noinline__ void eval_cell_direct(const ThetaC<T>& c, const GridC& g, const PolyTab<T>& btab, const PolyTab<T>& Ftab,
@@ -498,10 +678,12 @@ __device__ __noinline__ void eval_cell_direct(const ThetaC<T>& c, const GridC& g
             st = g.bulge_profile == 1 ? jaffe_sigma_tilde(sx) : sigma_tilde(sx);
             jj = g.bulge_profile == 1 ? jaffe_jeans_J(sx, dc.NJ, dc.glx, dc.glw) : jeans_J(sx, dc.NJ, dc.glx, dc.glw);
         }
+        if (has_ext(g))                                              // reading U'
+            jj += ext_Itilde<double, T>(sqrt(s2), c.d, ThetaF{}, g, Ftab, dc.quad);
         Bb = (double)c.ampBb * st;
         IbL = (double)c.ampIb * jj;
     }
-    const double vc2 = vc2_total<T>(c.d, g, Ftab, r);
+    const double vc2 = vc2_total<T>(c.d, g, g.comps, Ftab, r);
     // discs, with the common factor 2^shift taken out of the exponentials (no bulge: the ratios survive underflow)
     const double e1a = r * (double)c.cexp[0], e2a = r * (double)c.cexp[1];
     double shift = 0.0;
@@ -532,7 +714,7 @@ BANG_D EvalWalk make_walk(const int tid, const int NT, const int nfx) {
     return w;
 }
 template <typename T, bool BULGE, int SHIFT, bool FLUX>
-BANG_D void eval_rows(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab, T* __restrict__ dst,
+BANG_D void eval_rows(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs, const T* __restrict__ vtab, T* __restrict__ dst,
                       const size_t row_pitch, const size_t obs_stride, const int nfx, const int jy0, const int n_rows,
                       const EvalWalk& w, const int NT) {
     const int step_j = w.step_j, step_x = w.step_x;
@@ -542,7 +724,7 @@ BANG_D void eval_rows(const CellK<T>& k, const T* __restrict__ bbase, const T* _
     for (int i = tid; i < n; i += NT) {
         T vB, vV, vS, vL, xp, yp;
         rotate_cell<T>(k, (T)(x - k.jcx), (T)(jy0 + j - k.jcy), xp, yp);
-        eval_cell<T, BULGE, SHIFT, FLUX>(k, bbase, vtab, xp, yp, vB, vV, vS, vL);
+        eval_cell<T, BULGE, SHIFT, FLUX>(k, bbase, bs, vtab, xp, yp, vB, vV, vS, vL);
         T* d = dst + (size_t)j * row_pitch + x;
         d[0] = vB; d[obs_stride] = vV; d[2 * obs_stride] = vS; d[3 * obs_stride] = vL;
         x += step_x; j += step_j;
@@ -550,21 +732,21 @@ BANG_D void eval_rows(const CellK<T>& k, const T* __restrict__ bbase, const T* _
     }
 }
 template <typename T, bool FLUX>
-BANG_D void eval_rows_comps(const unsigned comps, const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab,
+BANG_D void eval_rows_comps(const unsigned comps, const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs, const T* __restrict__ vtab,
                             T* __restrict__ dst, const size_t row_pitch, const size_t obs_stride, const int nfx,
                             const int jy0, const int n_rows, const EvalWalk& w, const int NT) {
-    if (comps & C_BULGE) eval_rows<T, true, 0, FLUX>(k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    if (comps & C_BULGE) eval_rows<T, true, 0, FLUX>(k, bbase, bs, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_rows<T, false, 3, FLUX>(k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
-    else if (comps & C_DISC1) eval_rows<T, false, 1, FLUX>(k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
-    else eval_rows<T, false, 2, FLUX>(k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+        eval_rows<T, false, 3, FLUX>(k, bbase, bs, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else if (comps & C_DISC1) eval_rows<T, false, 1, FLUX>(k, bbase, bs, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else eval_rows<T, false, 2, FLUX>(k, bbase, bs, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
 }
 template <typename T>
-BANG_D void eval_rows_any(const unsigned comps, const bool flux, const CellK<T>& k, const T* __restrict__ bbase,
+BANG_D void eval_rows_any(const unsigned comps, const bool flux, const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs,
                           const T* __restrict__ vtab, T* __restrict__ dst, const size_t row_pitch, const size_t obs_stride,
                           const int nfx, const int jy0, const int n_rows, const EvalWalk& w, const int NT) {
-    if (flux) eval_rows_comps<T, true>(comps, k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
-    else eval_rows_comps<T, false>(comps, k, bbase, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    if (flux) eval_rows_comps<T, true>(comps, k, bbase, bs, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
+    else eval_rows_comps<T, false>(comps, k, bbase, bs, vtab, dst, row_pitch, obs_stride, nfx, jy0, n_rows, w, NT);
 }
 // the same block of rows through the direct path (a theta flagged slow)
 template <typename T>
@@ -623,7 +805,7 @@ constexpr int lbc_blocks(int lbc, int P, bool f64) {
 // dst[(row * 4 + observable) * NFB + x].  GUARD: some of the S rows lie past the grid (zero-weight tap padding): they
 // are written as zeros.
 template <typename T, int S, int NFB, int GRP, int PADV, bool BULGE, int SHIFT, bool GUARD>
-BANG_D void eval_superrow(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab, T* __restrict__ dst,
+BANG_D void eval_superrow(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs, const T* __restrict__ vtab, T* __restrict__ dst,
                           const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
     const T b0 = (T)(jy0 - k.jcy);
     const T bx = fma(b0, k.hs, k.xp0), by = fma(b0, k.hc, k.yp0);
@@ -639,20 +821,20 @@ BANG_D void eval_superrow(const CellK<T>& k, const T* __restrict__ bbase, const 
                 vB = vV = vS = vL = T(0);
             } else {
                 const T xp = j == 0 ? px : fma((T)j, k.hs, px), yp = j == 0 ? py : fma((T)j, k.hc, py);
-                eval_cell<T, BULGE, SHIFT>(k, bbase, vtab, xp, yp, vB, vV, vS, vL);
+                eval_cell<T, BULGE, SHIFT>(k, bbase, bs, vtab, xp, yp, vB, vV, vS, vL);
             }
             d[(j * 4 + 0) * NFB] = vB; d[(j * 4 + 1) * NFB] = vV; d[(j * 4 + 2) * NFB] = vS; d[(j * 4 + 3) * NFB] = vL;
         }
     }
 }
 template <typename T, int S, int NFB, int GRP, int PADV, bool GUARD>
-BANG_D void eval_superrow_any(const unsigned comps, const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ vtab,
+BANG_D void eval_superrow_any(const unsigned comps, const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs, const T* __restrict__ vtab,
                               T* __restrict__ dst, const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
-    if (comps & C_BULGE) eval_superrow<T, S, NFB, GRP, PADV, true, 0, GUARD>(k, bbase, vtab, dst, nfx, nfy, jy0, vt, NT);
+    if (comps & C_BULGE) eval_superrow<T, S, NFB, GRP, PADV, true, 0, GUARD>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_superrow<T, S, NFB, GRP, PADV, false, 3, GUARD>(k, bbase, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else if (comps & C_DISC1) eval_superrow<T, S, NFB, GRP, PADV, false, 1, GUARD>(k, bbase, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else eval_superrow<T, S, NFB, GRP, PADV, false, 2, GUARD>(k, bbase, vtab, dst, nfx, nfy, jy0, vt, NT);
+        eval_superrow<T, S, NFB, GRP, PADV, false, 3, GUARD>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else if (comps & C_DISC1) eval_superrow<T, S, NFB, GRP, PADV, false, 1, GUARD>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else eval_superrow<T, S, NFB, GRP, PADV, false, 2, GUARD>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
 }
 
 // ---- the fused kernel ---------------------------------------------------------------------------------------------
@@ -661,6 +843,8 @@ struct FusedParams {
     GridC g;
     FitC fit;
     PolyTab<T> btab, Ftab;
+    QuadC quad;                  // reading U': the N_J-node rule for Itilde_ext
+    int bs_elems;                // size of the per-theta bulge tables in shared memory, in values of T (bs_elems<T>(g))
     T W[NACC * S];               // composite x s box (*) Gaussian taps, zero padded (a4 + a5)
     const double* theta;         // [B][17]
     int B;
@@ -676,9 +860,15 @@ struct FusedParams {
 
 template <typename T>
 inline size_t vtab_bytes() { return ((size_t)kVcOct * (1 << TabCfg<T>::M) + 1) * (TabCfg<T>::D + 1) * sizeof(T); }
+// scratch for the nodes of Itilde_ext: the row buffer serves when there is one (k_fused), else (k_fine) it is allocated
 template <typename T>
-inline size_t fused_smem_bytes(int S, int nfb) {
-    return (sizeof(ThetaC<T>) + 15) / 16 * 16 + vtab_bytes<T>() + (size_t)S * 4 * nfb * sizeof(T) + 32 * sizeof(double);
+inline size_t ext_scratch_elems(const GridC& g) {
+    return has_ext(g) ? ((size_t)kBOct * (1 << TabCfg<T>::M)) * (TabCfg<T>::D + 1) + 4 : 0;
+}
+template <typename T>
+inline size_t fused_smem_bytes(const GridC& g, int S, int nfb) {
+    const size_t row = (size_t)S * 4 * nfb, scr = ext_scratch_elems<T>(g);
+    return (sizeof(ThetaC<T>) + 15) / 16 * 16 + vtab_bytes<T>() + (bs_elems<T>(g) + (row > scr ? row : scr)) * sizeof(T) + 32 * sizeof(double);
 }
 
 // N consecutive values from shared memory into registers with the widest vector loads the alignment ALIGN (bytes)
@@ -732,7 +922,9 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
     ThetaC<T>& c = *reinterpret_cast<ThetaC<T>*>(smem_raw);
     constexpr size_t off_tab = (sizeof(ThetaC<T>) + 15) / 16 * 16;
     T* vtab = reinterpret_cast<T*>(smem_raw + off_tab);
-    T* rowbuf = vtab + ((size_t)kVcOct * (1 << TabCfg<T>::M) + 1) * NC;
+    T* bs_mem = vtab + ((size_t)kVcOct * (1 << TabCfg<T>::M) + 1) * NC;
+    T* rowbuf = bs_mem + p.bs_elems;
+    const T* bs = p.bs_elems ? bs_mem : nullptr;
     constexpr int nfb = lbc_nfb(LBC, P, S, NACC, (int)sizeof(T));
     constexpr int GRP = P * S, PADV = row_pad(P, S, (int)sizeof(T));
     double* red = reinterpret_cast<double*>(rowbuf + (size_t)S * 4 * nfb);
@@ -753,7 +945,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
 
     for (int b = blockIdx.x; b < p.B; b += gridDim.x) {
         __syncthreads();
-        if (tid == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.Ftab, c);
+        if (tid == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.btab, p.Ftab, c);
         __syncthreads();
         if (!c.valid || (c.slow && !p.slow_list)) {  // out-of-domain theta: NaN maps / -inf likelihood
             if constexpr (MODE == 0) {
@@ -769,6 +961,13 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
             continue;
         }
         build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
+        if (p.bs_elems) {
+            build_bulge_tables<T>(c, g, p.fit, p.btab, p.Ftab, p.quad, bs_mem, rowbuf);
+            if (has_ext(g)) {                         // the row buffer served as scratch: zero the tap padding again
+                for (int i = tid; i < S * 4 * nfb; i += NT) rowbuf[i] = T(0);
+                __syncthreads();
+            }
+        }
 
         T acc[P][NACC];
 #pragma unroll
@@ -783,8 +982,8 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
             // the per-theta constants are re-read from shared memory for every super-row (a handful of broadcast loads)
             // so that they do not occupy registers during the PSF phase
             const CellK<T> k = load_cellk<T>(c);
-            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, GRP, PADV, false>(g.comps, k, bbase, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
-            else eval_superrow_any<T, S, nfb, GRP, PADV, true>(g.comps, k, bbase, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, GRP, PADV, false>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            else eval_superrow_any<T, S, nfb, GRP, PADV, true>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
             vt = vt + 32 < NT ? vt + 32 : vt + 32 - NT;      // rotate the column ownership by one warp: the ragged last
                                                              // pass then falls on a different warp (scheduler) each time
             __syncthreads();
@@ -859,6 +1058,7 @@ struct FineParams {
     FitC fit;
     PolyTab<T> btab, Ftab;
     DirectC direct;
+    int bs_elems;                // as in FusedParams
     const double* theta;
     int B;
     T* fine;                     // [B][4][nfy][nfx]
@@ -871,12 +1071,15 @@ __global__ void __launch_bounds__(256) k_fine(const __grid_constant__ FineParams
     ThetaC<T>& c = *reinterpret_cast<ThetaC<T>*>(smem_raw);
     constexpr size_t off_tab = (sizeof(ThetaC<T>) + 15) / 16 * 16;
     T* vtab = reinterpret_cast<T*>(smem_raw + off_tab);
+    T* bs_mem = vtab + ((size_t)kVcOct * (1 << TabCfg<T>::M) + 1) * NC;
+    T* scratch = bs_mem + p.bs_elems;
+    const T* bs = p.bs_elems ? bs_mem : nullptr;
     const GridC& g = p.g;
     const size_t plane = (size_t)g.nfx * g.nfy;
     const T* bbase = p.btab.coef - (ptrdiff_t)p.btab.first * (2 * NC);
     for (int b = blockIdx.x; b < p.B; b += gridDim.x) {
         __syncthreads();
-        if (threadIdx.x == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.Ftab, c);
+        if (threadIdx.x == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.btab, p.Ftab, c);
         __syncthreads();
         T* out = p.fine + (size_t)b * 4 * plane;
         if (!c.valid) {
@@ -891,7 +1094,8 @@ __global__ void __launch_bounds__(256) k_fine(const __grid_constant__ FineParams
             continue;
         }
         build_vc_table<T>(c, g, p.fit, p.Ftab, vtab);
-        eval_rows_any<T>(g.comps, g.flux != 0, k, bbase, vtab, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy,
+        if (p.bs_elems) build_bulge_tables<T>(c, g, p.fit, p.btab, p.Ftab, p.direct.quad, bs_mem, scratch);
+        eval_rows_any<T>(g.comps, g.flux != 0, k, bbase, bs, vtab, out, (size_t)g.nfx, plane, g.nfx, 0, g.nfy,
                          make_walk(threadIdx.x, blockDim.x, g.nfx), blockDim.x);
     }
 }

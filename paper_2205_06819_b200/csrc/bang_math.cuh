@@ -304,27 +304,31 @@ BANG_HD double nfw_r200(double M200) {
 // table has 2^M equal sub-intervals per octave of u, the interval number is the top bits (exponent and M mantissa bits)
 // and the position inside the interval, mapped to t in [-1, 1), is the remaining mantissa bits.  No logarithm is taken.
 // Every table stores, per interval, the D+1 coefficients of a polynomial in t (Chebyshev-node interpolant, monomial
-// form): D = 3, M = 4 in fp32 mode (relative error ~2e-7), D = 7, M = 3 in fp64 mode (~1e-11).
+// form): D = 3, M = 3 in fp32 mode (8 cubics per octave: relative error 4e-6 for SigmaTilde, 8e-6 for J, 6e-7 for F,
+// 2e-7 for v_c -- measured against direct evaluation; the mode's tolerance is 1e-4), D = 7, M = 3 in fp64 mode (~1e-11).
+// Round 1 used M = 4 in fp32 mode (3e-7): halving the tables is what lets the theta's slice of the bulge table live in
+// shared memory next to its v_c table.
 template <typename T> struct TabCfg;
-template <> struct TabCfg<float>  { static constexpr int D = 3, M = 4; };
+template <> struct TabCfg<float>  { static constexpr int D = 3, M = 3; };
 template <> struct TabCfg<double> { static constexpr int D = 7, M = 3; };
 
 // global interval number of u (before subtracting the table's first interval): (biased exponent << M) | top mantissa bits
 BANG_HD int tab_cell(float u, float& t) {
+    constexpr int M = TabCfg<float>::M, LOW = 23 - M;
 #if defined(__CUDA_ARCH__)
     const int bits = __float_as_int(u);
-    // tau = 1 + (low 19 mantissa bits) 2^-23 in [1, 1 + 2^-4);  t = 32 tau - 33, exact: one LOP3 and one FFMA
-    // (both masks as register operands, or ptxas splits (bits & m) | c into two LOP3 with one immediate each)
+    // tau = 1 + (low 23-M mantissa bits) 2^-23 in [1, 1 + 2^-M);  t = 2^(M+1) tau - (2^(M+1) + 1), exact: one LOP3 and one
+    // FFMA (both masks as register operands, or ptxas splits (bits & m) | c into two LOP3 with one immediate each)
     int tau;
-    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(tau) : "r"(bits), "r"(0x7FFFF), "r"(0x3F800000));
-    t = fmaf(__int_as_float(tau), 32.0f, -33.0f);
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(tau) : "r"(bits), "r"((1 << LOW) - 1), "r"(0x3F800000));
+    t = fmaf(__int_as_float(tau), (float)(2 << M), -(float)((2 << M) + 1));
 #else
     union { float f; int i; } c; c.f = u;
     const int bits = c.i;
-    union { int i; float f; } d; d.i = ((bits & 0x7FFFF) << 4) | 0x40000000;
+    union { int i; float f; } d; d.i = ((bits & ((1 << LOW) - 1)) << M) | 0x40000000;
     t = d.f - 3.0f;
 #endif
-    return bits >> 19;                                   // 23 - M, M = 4
+    return bits >> LOW;
 }
 BANG_HD int tab_cell(double u, double& t) {
 #if defined(__CUDA_ARCH__)
@@ -340,7 +344,7 @@ BANG_HD int tab_cell(double u, double& t) {
 }
 // first global interval number of the octave 2^e
 template <typename T> BANG_HD int tab_first_cell(int e);
-template <> BANG_HD int tab_first_cell<float>(int e) { return (e + 127) << 4; }
+template <> BANG_HD int tab_first_cell<float>(int e) { return (e + 127) << TabCfg<float>::M; }
 template <> BANG_HD int tab_first_cell<double>(int e) { return (e + 1023) << 3; }
 
 // lower edge and width of interval `cell` (global number), as doubles

@@ -85,11 +85,11 @@ __global__ void k_moments_reduce(const double* __restrict__ chi2, const int* __r
 }
 // validity of each theta of a chunk (the decode's verdict), for the kernels above
 template <typename T>
-__global__ void k_theta_valid(const double* __restrict__ theta, int Bc, GridC g, PolyTab<T> Ftab, int* __restrict__ valid) {
+__global__ void k_theta_valid(const double* __restrict__ theta, int Bc, GridC g, PolyTab<T> btab, PolyTab<T> Ftab, int* __restrict__ valid) {
     const int bl = blockIdx.x * blockDim.x + threadIdx.x;
     if (bl >= Bc) return;
     ThetaC<T> c;
-    decode_theta<T>(theta + (size_t)bl * kNTheta, g, Ftab, c);
+    decode_theta<T>(theta + (size_t)bl * kNTheta, g, btab, Ftab, c);
     valid[bl] = c.valid;
 }
 
