@@ -63,8 +63,9 @@ extern "C" {
 #define BANG_PSF_FIELDS 0        /* the paper: eq. 21 applied to B, v_los, sigma_los, <L/M> separately (reading G) */
 #define BANG_PSF_FLUX   1        /* variant (reading G'): PSF + rebin applied to the light moments B, B v, B (sigma^2 + v^2)
                                     and to the mass surface density; v = M1/M0, sigma^2 = M2/M0 - v^2, M/L = M3/M0.
-                                    bang_model_fine then returns those four moment fields.  A side variant, run UNFUSED
-                                    (moment fields through HBM scratch, several kernels per call), not the tuned path */
+                                    bang_model_fine then returns those four moment fields.  Runs in the fused kernel (its
+                                    own instantiation: the four moments of a pixel meet by warp shuffle when its row
+                                    completes) */
 #define BANG_POTENTIAL_SELF  0    /* the paper: the bulge's dispersion in its own potential, eq. 6 */
 #define BANG_POTENTIAL_TOTAL 1    /* variant (reading U'; PAPER.md:417-419 names the approximation above as the model's first
                                     limitation): Sigma_b sigma_b^2 gains I_ext(R) = 2 int_R^inf rho_b v_ext^2 sqrt(x^2-R^2)/x dx,
@@ -139,6 +140,24 @@ int bang_model_fine(bang_ctx *ctx, const double *theta_dev, int B, void *fine_de
  * gives -inf (a nested sampler treats it as zero likelihood).  BANG_ENODATA before bang_set_data.
  * Asynchronous. */
 int bang_loglike(bang_ctx *ctx, const double *theta_dev, int B, double *logL_dev);
+
+/* The replacement step of nested sampling on the device (the worst live point is
+ * replaced by one of higher likelihood found by MCMC): K constrained random walks of `steps` Metropolis steps in lock-step,
+ * each step = proposal kernel -> bang_loglike on the K proposals -> accept kernel, with walkers, proposals and their
+ * parameter vectors resident in device memory throughout (one small host<->device exchange per CALL, none per step).
+ * Walkers live in the unit cube u in [0,1]^d (uniform prior); theta = theta0 with theta[free_idx[j]] = lo[j] + (hi[j] -
+ * lo[j]) u[j].  Walker k belongs to group[k] in [0, n_groups) -- one group per independent run or retire batch, so that
+ * several of them share one call and fill the GPU: a proposal is u + scale[g] (2.38/sqrt d) chol[g] z, z ~ N(0, 1)^d
+ * (Philox4x32-10, counter = (walker, step, draw), key = seed), accepted iff it stays in the cube and its logL exceeds
+ * Lstar[k] (out-of-domain theta: logL = -inf, never accepted).
+ * HOST: free_idx[d], lo[d], hi[d], theta0[17], chol[n_groups][d][d] (lower triangular, row-major), scale[n_groups],
+ * n_accept[n_groups] (out: accepted proposals per group).  DEVICE: u [K][d] and logL [K] (in/out: the walkers and their
+ * likelihoods), Lstar [K], group [K].  d <= 17.  Synchronises the stream before returning.  BANG_ENODATA before
+ * bang_set_data; BANG_EINVAL on bad sizes or NULL pointers. */
+int bang_ns_walk(bang_ctx *ctx, int K, int d, const int *free_idx_host, const double *lo_host, const double *hi_host,
+                 const double *theta0_host, double *u_dev, double *logL_dev, const double *Lstar_dev, const int *group_dev,
+                 int n_groups, const double *chol_host, const double *scale_host, int steps, unsigned long long seed,
+                 int *n_accept_host);
 
 /* Same calls with HOST buffers: the library stages theta in pinned memory, copies it to the device, runs, and copies
  * the result back; synchronises the stream before returning.  logL_host [B] doubles; maps_host as maps_dev above. */

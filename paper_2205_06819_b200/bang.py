@@ -21,11 +21,12 @@ FP32, FP64 = 0, 1
 PSF_FIELDS, PSF_FLUX = 0, 1
 POTENTIAL_SELF, POTENTIAL_TOTAL = 0, 1
 HAS_TOTAL_POTENTIAL = True        # bench.py's sweep row for reading U'
+FLUX_IS_FUSED = True              # reading G' runs inside k_fused (bench.py then reports its roofline)
 NTHETA = 17
 OK, EINVAL, ENOMEM, ECUDA, ENODATA = 0, -1, -2, -3, -4
 
 EXPORTS = ["bang_create", "bang_set_data", "bang_model_maps", "bang_model_fine", "bang_loglike", "bang_loglike_host",
-           "bang_model_maps_host", "bang_get_geometry", "bang_launch_count", "bang_probe_peaks", "bang_ml_from_colour", "bang_destroy", "bang_strerror",
+           "bang_model_maps_host", "bang_ns_walk", "bang_get_geometry", "bang_launch_count", "bang_probe_peaks", "bang_ml_from_colour", "bang_destroy", "bang_strerror",
            "bang_last_error"]
 
 
@@ -74,6 +75,8 @@ def lib():
         L.bang_probe_peaks.argtypes, L.bang_probe_peaks.restype = [vp, C.POINTER(C.c_double)], ip
         L.bang_ml_from_colour.argtypes = [vp, vp, vp, vp, C.c_longlong, dp, dp, dp, vp, vp, ip, vp]
         L.bang_ml_from_colour.restype = ip
+        L.bang_ns_walk.argtypes = [vp, ip, ip, vp, vp, vp, vp, vp, vp, vp, vp, ip, vp, vp, ip, C.c_ulonglong, vp]
+        L.bang_ns_walk.restype = ip
         L.bang_destroy.argtypes, L.bang_destroy.restype = [vp], None
         L.bang_strerror.argtypes, L.bang_strerror.restype = [ip], C.c_char_p
         L.bang_last_error.argtypes, L.bang_last_error.restype = [vp], C.c_char_p
@@ -199,6 +202,32 @@ class Context:
             out = np.empty(B, dtype=np.float64)
         self._check(lib().bang_loglike_host(self._h, t.ctypes.data, B, out.ctypes.data))
         return out
+
+    def ns_walk(self, u, logL, Lstar, group, chol, scale, free, lo, hi, theta0, steps: int, seed: int = 0) -> np.ndarray:
+        """bang_ns_walk: advance the walkers u [K][d] (float64 device tensor, updated in place together with logL [K])
+        by `steps` constrained Metropolis steps on the device.  Lstar [K] float64 and group [K] int32 device tensors;
+        chol [G][d][d], scale [G], free [d], lo [d], hi [d], theta0 [17] host arrays.  Returns the accepted proposals per
+        group (host int array); synchronises."""
+        torch = self._torch
+        K, d = u.shape
+        chol = np.ascontiguousarray(chol, dtype=np.float64)
+        G = chol.shape[0]
+        assert chol.shape == (G, d, d) and u.dtype == torch.float64 and logL.dtype == torch.float64
+        assert Lstar.dtype == torch.float64 and group.dtype == torch.int32 and u.is_contiguous()
+        assert u.device == logL.device == Lstar.device == group.device == self.device
+        scale = np.ascontiguousarray(scale, dtype=np.float64).reshape(G)
+        free = np.ascontiguousarray(free, dtype=np.int32).reshape(d)
+        lo = np.ascontiguousarray(lo, dtype=np.float64).reshape(d)
+        hi = np.ascontiguousarray(hi, dtype=np.float64).reshape(d)
+        theta0 = np.ascontiguousarray(theta0, dtype=np.float64).reshape(NTHETA)
+        n_acc = np.zeros(G, dtype=np.int32)
+        self._stream.wait_stream(torch.cuda.current_stream(self.device))    # the caller filled the tensors on its stream
+        with self._on_stream():
+            self._check(lib().bang_ns_walk(self._h, K, d, free.ctypes.data, lo.ctypes.data, hi.ctypes.data, theta0.ctypes.data,
+                                           u.data_ptr(), logL.data_ptr(), Lstar.data_ptr(), group.data_ptr(), G,
+                                           chol.ctypes.data, scale.ctypes.data, int(steps), int(seed) & (2**64 - 1),
+                                           n_acc.ctypes.data))
+        return n_acc
 
     def probe_peaks(self) -> dict:
         """Measured sustained instruction rates [thread-instr/s] of dependency-free FFMA, MUFU.EX2 and DFMA chains."""

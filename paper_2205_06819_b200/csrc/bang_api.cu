@@ -9,7 +9,7 @@
 
 #include "../../include/bang.h"
 #include "bang_host.h"
-#include "bang_moments.cuh"
+#include "bang_ns.cuh"
 #include "bang_slow.cuh"
 
 using namespace bang;
@@ -40,9 +40,10 @@ struct bang_ctx {
     // direct path (bang_slow.cuh): list of the theta k_fused leaves to k_slow, {count, CTAs done}, capacity; 0 = the grid
     // is too large for k_slow's shared memory (such theta are then reported as out of domain)
     int* slow_list = nullptr; int* slow_cnt = nullptr; int slow_cap = 0; size_t slow_smem = 0;
-    // flux-weighted PSF variant (unfused): composite taps on the device, scratch for the moment fields of a chunk of theta
-    double* W_dev = nullptr; void* fx_fine = nullptr; int* fx_valid = nullptr; double* fx_chi2 = nullptr;
-    int fx_chunk = 0; size_t fx_chi2_cap = 0;          // per mode: resident CTAs per SM once the kernel is configured
+    double* W_dev = nullptr;               // composite taps on the device (direct path)
+    // bang_ns_walk scratch: proposals [K][d], their theta [K][17] and likelihoods [K], Cholesky factors + scales, counts
+    double* ns_prop = nullptr; double* ns_theta = nullptr; double* ns_pl = nullptr; double* ns_chol = nullptr;
+    int* ns_acc = nullptr; int ns_capK = 0, ns_capG = 0;
     char err[512] = {0};
 };
 
@@ -283,7 +284,19 @@ cudaError_t dispatch_fused(const bang_ctx* c, const FusedLaunch& L, FusedInfo* i
     }
 }
 
-QuadC make_quad(const bang_ctx* c) { return QuadC{c->qd_dev, c->qf_dev, c->model.jeans_nodes}; }
+QuadC make_quad(const bang_ctx* c) {
+    QuadC q{};
+    q.qd = c->qd_dev; q.qf = c->qf_dev; q.NJ = c->model.jeans_nodes;
+    // coarse panels of the per-theta Itilde_ext build (bang_kernels.cuh): 8 nodes per 2 octaves in fp32 mode, 12 per octave in fp64
+    q.ND = c->model.precision == BANG_FP64 ? 12 : 8;
+    q.span = c->model.precision == BANG_FP64 ? 1 : 2;
+    for (int k = 0; k < q.ND; ++k) {
+        const long double a = 3.14159265358979323846264338328L * (2 * k + 1) / (2.0L * q.ND);
+        q.bx[k] = (double)cosl(a);
+        q.bw[k] = (double)((k & 1 ? -1.0L : 1.0L) * sinl(a));
+    }
+    return q;
+}
 DirectC make_direct(const bang_ctx* c) {
     return DirectC{c->gl_dev, c->gl_dev + c->model.jeans_nodes, c->model.jeans_nodes, make_quad(c)};
 }
@@ -366,47 +379,6 @@ int ensure_staging(bang_ctx* ctx, int B, size_t out_bytes) {
         CU(cudaMallocHost(&ctx->h_out, out_bytes));
         CU(cudaMalloc(&ctx->d_out, out_bytes));
         ctx->cap_out = out_bytes;
-    }
-    return BANG_OK;
-}
-
-// BANG_PSF_FLUX: k_fine (moment fields of a chunk of theta -> HBM scratch) + k_psf_moments (+ k_moments_reduce)
-template <typename T>
-int run_flux(bang_ctx* ctx, const double* theta_dev, int B, int mode, void* maps_dev, double* logL_dev) {
-    const GridC& g = ctx->g;
-    const size_t plane4 = (size_t)4 * g.nfx * g.nfy * sizeof(T);
-    const int ntap = 2 * ctx->rk + g.s;
-    if (!ctx->fx_fine) {                                              // scratch: at most 256 MiB of moment fields
-        ctx->fx_chunk = (int)std::max<size_t>(1, std::min<size_t>(4096, ((size_t)256 << 20) / plane4));
-        CU(cudaMalloc(&ctx->fx_fine, (size_t)ctx->fx_chunk * plane4));
-        CU(cudaMalloc(&ctx->fx_valid, (size_t)ctx->fx_chunk * sizeof(int)));
-    }
-    if (mode == 1 && (size_t)B * g.ny > ctx->fx_chi2_cap) {
-        cudaFree(ctx->fx_chi2); ctx->fx_chi2 = nullptr; ctx->fx_chi2_cap = 0;
-        CU(cudaMalloc(&ctx->fx_chi2, (size_t)B * g.ny * sizeof(double)));
-        ctx->fx_chi2_cap = (size_t)B * g.ny;
-    }
-    const size_t smem = fused_smem_bytes<T>(g, 0, 0);
-    CU(cudaFuncSetAttribute(k_fine<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const int gmax = data_gmax(ctx);
-    const DirectC direct = make_direct(ctx);
-    for (int b0 = 0; b0 < B; b0 += ctx->fx_chunk) {
-        const int Bc = std::min(ctx->fx_chunk, B - b0);
-        const double* th = theta_dev + (size_t)b0 * kNTheta;
-        const PolyTab<T> Ft{static_cast<const T*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells};
-        const PolyTab<T> Bt{static_cast<const T*>(ctx->btab), ctx->btab_first, ctx->btab_cells};
-        k_theta_valid<T><<<(Bc + 127) / 128, 128, 0, ctx->stream>>>(th, Bc, g, Bt, Ft, ctx->fx_valid);
-        FineParams<T> fp{g, ctx->fit, Bt, Ft, direct, (int)bs_elems<T>(g), th, Bc, static_cast<T*>(ctx->fx_fine)};
-        k_fine<T><<<std::min(Bc, 8 * ctx->n_sm), 256, smem, ctx->stream>>>(fp);
-        MomentsParams<T> mp{g, ntap, ctx->W_dev, static_cast<const T*>(ctx->fx_fine), Bc, b0, ctx->fx_valid,
-                            static_cast<T*>(maps_dev), ctx->data, ctx->P, gmax, ctx->fx_chi2, mode};
-        k_psf_moments<T><<<Bc * g.ny, 128, 0, ctx->stream>>>(mp);
-        ctx->launches += 3;
-        if (mode == 1) {
-            k_moments_reduce<<<(Bc + 127) / 128, 128, 0, ctx->stream>>>(ctx->fx_chi2, ctx->fx_valid, Bc, b0, g.ny, ctx->C0, logL_dev);
-            ctx->launches += 1;
-        }
-        CU(cudaGetLastError());
     }
     return BANG_OK;
 }
@@ -494,7 +466,8 @@ void bang_destroy(bang_ctx* ctx) {
     cudaFree(ctx->btab); cudaFree(ctx->Ftab); cudaFree(ctx->data); cudaFree(ctx->scal); cudaFree(ctx->gl_dev); cudaFree(ctx->qd_dev); cudaFree(ctx->qf_dev);
     cudaFree(ctx->d_theta); cudaFree(ctx->d_out);
     cudaFree(ctx->slow_list); cudaFree(ctx->slow_cnt);
-    cudaFree(ctx->W_dev); cudaFree(ctx->fx_fine); cudaFree(ctx->fx_valid); cudaFree(ctx->fx_chi2);
+    cudaFree(ctx->W_dev);
+    cudaFree(ctx->ns_prop); cudaFree(ctx->ns_theta); cudaFree(ctx->ns_pl); cudaFree(ctx->ns_chol); cudaFree(ctx->ns_acc);
     if (ctx->h_theta) cudaFreeHost(ctx->h_theta);
     if (ctx->h_out) cudaFreeHost(ctx->h_out);
     delete ctx;
@@ -660,9 +633,6 @@ int bang_model_maps(bang_ctx* ctx, const double* theta_dev, int B, void* maps_de
     if (B < 0 || (B > 0 && (!theta_dev || !maps_dev))) return fail(ctx, BANG_EINVAL, "bang_model_maps: bad arguments");
     if (B == 0) return BANG_OK;
     ON_DEVICE(ctx);
-    if (ctx->model.psf_weighting == BANG_PSF_FLUX)
-        return ctx->model.precision == BANG_FP64 ? run_flux<double>(ctx, theta_dev, B, 0, maps_dev, nullptr)
-                                                 : run_flux<float>(ctx, theta_dev, B, 0, maps_dev, nullptr);
     int rc = ensure_slow_list(ctx, B);
     if (rc != BANG_OK) return rc;
     FusedLaunch L = make_launch(ctx, theta_dev, B, 0, maps_dev, nullptr);
@@ -678,9 +648,6 @@ int bang_loglike(bang_ctx* ctx, const double* theta_dev, int B, double* logL_dev
     if (!ctx->has_data) return fail(ctx, BANG_ENODATA, "bang_loglike: no data loaded");
     if (B == 0) return BANG_OK;
     ON_DEVICE(ctx);
-    if (ctx->model.psf_weighting == BANG_PSF_FLUX)
-        return ctx->model.precision == BANG_FP64 ? run_flux<double>(ctx, theta_dev, B, 1, nullptr, logL_dev)
-                                                 : run_flux<float>(ctx, theta_dev, B, 1, nullptr, logL_dev);
     int rc = ensure_slow_list(ctx, B);
     if (rc != BANG_OK) return rc;
     FusedLaunch L = make_launch(ctx, theta_dev, B, 1, nullptr, logL_dev);
@@ -688,6 +655,66 @@ int bang_loglike(bang_ctx* ctx, const double* theta_dev, int B, double* logL_dev
     ctx->launches += 1;
     return ctx->model.precision == BANG_FP64 ? run_slow<double>(ctx, theta_dev, 1, nullptr, logL_dev)
                                              : run_slow<float>(ctx, theta_dev, 1, nullptr, logL_dev);
+}
+
+int bang_ns_walk(bang_ctx* ctx, int K, int d, const int* free_idx_host, const double* lo_host, const double* hi_host,
+                 const double* theta0_host, double* u_dev, double* logL_dev, const double* Lstar_dev, const int* group_dev,
+                 int n_groups, const double* chol_host, const double* scale_host, int steps, unsigned long long seed,
+                 int* n_accept_host) {
+    if (!ctx) return BANG_EINVAL;
+    if (K < 0 || d < 1 || d > kNsMaxDim || n_groups < 1 || steps < 0 || !free_idx_host || !lo_host || !hi_host || !theta0_host ||
+        !chol_host || !scale_host || !n_accept_host || (K > 0 && (!u_dev || !logL_dev || !Lstar_dev || !group_dev)))
+        return fail(ctx, BANG_EINVAL, "bang_ns_walk: bad arguments");
+    for (int j = 0; j < d; ++j)
+        if (free_idx_host[j] < 0 || free_idx_host[j] >= kNTheta) return fail(ctx, BANG_EINVAL, "bang_ns_walk: free index out of range");
+    if (!ctx->has_data) return fail(ctx, BANG_ENODATA, "bang_ns_walk: no data loaded");
+    for (int g = 0; g < n_groups; ++g) n_accept_host[g] = 0;
+    if (K == 0 || steps == 0) return BANG_OK;
+    ON_DEVICE(ctx);
+    if (K > ctx->ns_capK) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->ns_prop); cudaFree(ctx->ns_theta); cudaFree(ctx->ns_pl);
+        ctx->ns_prop = ctx->ns_theta = ctx->ns_pl = nullptr; ctx->ns_capK = 0;
+        CU(cudaMalloc(&ctx->ns_prop, (size_t)K * kNsMaxDim * sizeof(double)));
+        CU(cudaMalloc(&ctx->ns_theta, (size_t)K * kNTheta * sizeof(double)));
+        CU(cudaMalloc(&ctx->ns_pl, (size_t)K * sizeof(double)));
+        ctx->ns_capK = K;
+    }
+    if (n_groups > ctx->ns_capG) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->ns_chol); cudaFree(ctx->ns_acc);
+        ctx->ns_chol = nullptr; ctx->ns_acc = nullptr; ctx->ns_capG = 0;
+        CU(cudaMalloc(&ctx->ns_chol, (size_t)n_groups * (kNsMaxDim * kNsMaxDim + 1) * sizeof(double)));
+        CU(cudaMalloc(&ctx->ns_acc, (size_t)n_groups * sizeof(int)));
+        ctx->ns_capG = n_groups;
+    }
+    // Cholesky factors then scales (times the random-walk Metropolis factor 2.38/sqrt(d)), one small synchronous copy
+    std::vector<double> cs((size_t)n_groups * d * d + n_groups);
+    memcpy(cs.data(), chol_host, (size_t)n_groups * d * d * sizeof(double));
+    for (int g = 0; g < n_groups; ++g) cs[(size_t)n_groups * d * d + g] = scale_host[g] * 2.38 / std::sqrt((double)d);
+    CU(cudaMemcpyAsync(ctx->ns_chol, cs.data(), cs.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));                          // cs is pageable host memory: done before it goes away
+    CU(cudaMemsetAsync(ctx->ns_acc, 0, (size_t)n_groups * sizeof(int), ctx->stream));
+    NsParams p{};
+    p.K = K; p.d = d; p.seed = seed;
+    for (int j = 0; j < d; ++j) { p.free_idx[j] = free_idx_host[j]; p.lo[j] = lo_host[j]; p.hi[j] = hi_host[j]; }
+    for (int i = 0; i < kNTheta; ++i) p.theta0[i] = theta0_host[i];
+    p.u = u_dev; p.logL = logL_dev; p.Lstar = Lstar_dev; p.group = group_dev;
+    p.chol = ctx->ns_chol; p.scale = ctx->ns_chol + (size_t)n_groups * d * d;
+    p.prop = ctx->ns_prop; p.theta = ctx->ns_theta;
+    const int th = 128, blocks = (K + th - 1) / th;
+    for (int step = 0; step < steps; ++step) {
+        p.step = step;
+        k_ns_propose<<<blocks, th, 0, ctx->stream>>>(p);
+        int rc = bang_loglike(ctx, ctx->ns_theta, K, ctx->ns_pl);
+        if (rc != BANG_OK) return rc;
+        k_ns_accept<<<blocks, th, 0, ctx->stream>>>(K, d, ctx->ns_prop, ctx->ns_pl, Lstar_dev, group_dev, u_dev, logL_dev, ctx->ns_acc);
+        ctx->launches += 2;
+    }
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(n_accept_host, ctx->ns_acc, (size_t)n_groups * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return BANG_OK;
 }
 
 int bang_model_fine(bang_ctx* ctx, const double* theta_dev, int B, void* fine_dev) {

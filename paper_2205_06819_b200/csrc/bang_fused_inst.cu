@@ -13,9 +13,9 @@
 namespace bang {
 namespace {
 
-template <typename T, int S, int NACC, int P, int MODE, int LBC>
+template <typename T, int S, int NACC, int P, int MODE, int LBC, bool FLUX>
 cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) {
-    auto kern = k_fused<T, S, NACC, P, MODE, LBC>;
+    auto kern = k_fused<T, S, NACC, P, MODE, LBC, FLUX>;
     if (L.threads > lbc_threads(LBC)) return cudaErrorInvalidValue;
     const size_t smem = fused_smem_bytes<T>(L.g, S, lbc_nfb(LBC, P, S, NACC, (int)sizeof(T)));
     // the shared-memory opt-in and the occupancy query are done once per context and mode (L.cache, owned by the
@@ -42,8 +42,8 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     if (getenv("BANG_VERBOSE")) {
         cudaFuncAttributes fa;
         cudaFuncGetAttributes(&fa, kern);
-        fprintf(stderr, "[bang] k_fused<%s,S=%d,NACC=%d,P=%d,MODE=%d,LBC=%d> regs=%d smem=%zu threads=%d ctas/SM=%d grid=%d B=%d\n",
-                sizeof(T) == 4 ? "f32" : "f64", S, NACC, P, MODE, LBC, fa.numRegs, smem, L.threads, per_sm, ctas, L.B);
+        fprintf(stderr, "[bang] k_fused<%s,S=%d,NACC=%d,P=%d,MODE=%d,LBC=%d,FLUX=%d> regs=%d smem=%zu threads=%d ctas/SM=%d grid=%d B=%d\n",
+                sizeof(T) == 4 ? "f32" : "f64", S, NACC, P, MODE, LBC, (int)FLUX, fa.numRegs, smem, L.threads, per_sm, ctas, L.B);
     }
 #endif
 
@@ -62,8 +62,11 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
 
 template <typename T, int S, int NACC, int P, int LBC>
 cudaError_t launch_lbc(const FusedLaunch& L, FusedInfo* info, bool query_only) {
-    return L.mode == 0 ? launch_mode<T, S, NACC, P, 0, LBC>(L, info, query_only)
-                       : launch_mode<T, S, NACC, P, 1, LBC>(L, info, query_only);
+    if (L.g.flux)      // reading G': a separate instantiation, so that the paper's path keeps its registers
+        return L.mode == 0 ? launch_mode<T, S, NACC, P, 0, LBC, true>(L, info, query_only)
+                           : launch_mode<T, S, NACC, P, 1, LBC, true>(L, info, query_only);
+    return L.mode == 0 ? launch_mode<T, S, NACC, P, 0, LBC, false>(L, info, query_only)
+                       : launch_mode<T, S, NACC, P, 1, LBC, false>(L, info, query_only);
 }
 template <typename T, int S, int NACC, int P>
 cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {

@@ -390,7 +390,14 @@ struct QuadC {
     const double2* qd;           // [N_J] {a_k, b_k} (device)
     const float2* qf;            // the same rounded to fp32
     int NJ;
+    // Itilde_ext is evaluated by the rule only at the ND Chebyshev nodes (in w = log2 s^2) of panels of `span` octaves and
+    // carried to the table's own nodes by barycentric interpolation of ln Itilde_ext(w) (measured on prior-drawn theta:
+    // 8 nodes per 2 octaves reproduce the rule to 8e-8, 12 nodes per octave to 6e-14): bx = the nodes on [-1,1], bw = the
+    // barycentric weights (-1)^k sin((2k+1) pi/(2 ND)).
+    int ND, span;
+    double bx[12], bw[12];
 };
+constexpr int kExtMaxND = 12;
 BANG_D void quad_node(const QuadC& q, int k, double& a, double& b) { const double2 v = __ldg(q.qd + k); a = v.x; b = v.y; }
 BANG_D void quad_node(const QuadC& q, int k, float& a, float& b) { const float2 v = __ldg(q.qf + k); a = v.x; b = v.y; }
 template <typename T>
@@ -443,36 +450,49 @@ BANG_D void build_bulge_tables(const ThetaC<T>& c, const GridC& g, const FitC& f
         for (int i = threadIdx.x; i < c.bcells * 2; i += blockDim.x) dst[2 + i] = __ldg(src + i);
     }
     if (!ext) { __syncthreads(); return; }
-    // Itilde_ext at the Chebyshev nodes of every interval of the slice (+ the nearest cell), then the fit
+    // Itilde_ext by the N_J-node rule at the coarse panel nodes (+ the nearest cell, directly), ...
     const int n = c.bcells * NC;
-    if constexpr (sizeof(T) == 4) {
+    const int octaves = c.bcells >> TabCfg<T>::M, panels = (octaves + q.span - 1) / q.span, ncoarse = panels * q.ND;
+    T* coarse = scratch + n + 4;                         // [panels][ND] ln Itilde_ext, then [ncoarse] = the nearest cell's value
+    const int e0 = (c.bfirst >> TabCfg<T>::M) - (sizeof(T) == 4 ? 127 : 1023);     // first octave of the slice
+    {
         const ThetaF df{(float)c.d.GMb, (float)c.d.Rb, {(float)c.d.Ad[0], (float)c.d.Ad[1]},
                         {(float)c.d.inv2Rd[0], (float)c.d.inv2Rd[1]}, (float)c.d.Ah, (float)c.d.hs};
-        for (int i = threadIdx.x; i <= n; i += blockDim.x) {
-            float s2;
-            if (i == n) s2 = (float)c.d.s2near;
-            else {
-                const int cell = i / NC, k = i - cell * NC;
-                double lo, width;
-                tab_interval<T>(c.bfirst + cell, lo, width);
-                s2 = (float)(lo + 0.5 * width * (fit.tnode[k] + 1.0));
-            }
-            scratch[i] = ext_Itilde<float, float>(sqrtf(s2), c.d, df, g, Ftab, q);
-        }
-    } else {
-        const ThetaF df{};
-        for (int i = threadIdx.x; i <= n; i += blockDim.x) {
+        for (int i = threadIdx.x; i <= ncoarse; i += blockDim.x) {
             double s2;
-            if (i == n) s2 = c.d.s2near;
+            if (i == ncoarse) s2 = c.d.s2near;
             else {
-                const int cell = i / NC, k = i - cell * NC;
-                double lo, width;
-                tab_interval<T>(c.bfirst + cell, lo, width);
-                s2 = lo + 0.5 * width * (fit.tnode[k] + 1.0);
+                const int pn = i / q.ND, k = i - pn * q.ND;
+                s2 = exp2((double)(e0 + pn * q.span) + 0.5 * q.span * (q.bx[k] + 1.0));
             }
-            scratch[i] = (T)ext_Itilde<double, T>(sqrt(s2), c.d, df, g, Ftab, q);
+            T v;
+            if constexpr (sizeof(T) == 4) v = ext_Itilde<float, float>(sqrtf((float)s2), c.d, df, g, Ftab, q);
+            else v = (T)ext_Itilde<double, T>(sqrt(s2), c.d, df, g, Ftab, q);
+            coarse[i] = i == ncoarse ? v : (T)log(fmax((double)v, 1e-300));
         }
     }
+    __syncthreads();
+    // ... then at the Chebyshev nodes of every interval of the slice by barycentric interpolation in w = log2 s^2
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const int cell = i / NC, k = i - cell * NC;
+        double lo, width;
+        tab_interval<T>(c.bfirst + cell, lo, width);
+        const double w = log2(lo + 0.5 * width * (fit.tnode[k] + 1.0));
+        const int pn = min((int)((w - e0) / q.span), panels - 1);
+        const double x = (w - (e0 + pn * q.span)) * (2.0 / q.span) - 1.0;
+        const T* gk = coarse + pn * q.ND;
+        double num = 0.0, den = 0.0, hit = 0.0;
+        bool exact = false;
+        for (int j = 0; j < q.ND; ++j) {
+            const double dx = x - q.bx[j];
+            if (dx == 0.0) { exact = true; hit = (double)gk[j]; }
+            const double wj = q.bw[j] / (dx == 0.0 ? 1.0 : dx);
+            num = fma(wj, (double)gk[j], num);
+            den += wj;
+        }
+        scratch[i] = (T)exp(exact ? hit : num / den);
+    }
+    if (threadIdx.x == 0) scratch[n] = coarse[ncoarse];
     __syncthreads();
     fit_cells<T>(fit, scratch, c.bcells);
     __syncthreads();
@@ -541,16 +561,20 @@ BANG_D void combine_cell(const CellK<T>& k, const T Bb, const T IbL, const T E1,
     const T invB = fast_rcp(Btot);
     const T kB = fma(k.vkB0, E1, k.vkB1 * E2);                              // sum_j B_d,j (-k_j sin i)
     const T qB = fma(k.q3B0, E1, k.q3B1 * E2);                              // sum_j B_d,j (1 - k_j^2)/3
-    oV = cosphi * vc * kB * invB;
-    oS = fast_sqrt(fma(vc * vc, qB, IbL) * invB);
-    oLM = Btot * fast_rcp(Stot);
-    oB = BULGE ? Btot : Btot * fast_exp2(shift);
     if constexpr (FLUX) {
-        // reading G': the PSF acts on the light moments B, B v, B (sigma^2 + v^2) and on the mass surface density B / <L/M>
-        const T v = oV;
-        oV = oB * v;
-        oS = oB * fma(oS, oS, v * v);
-        oLM = oB * fast_rcp(oLM);
+        // reading G': the PSF acts on the light moments B, B v, B (sigma^2 + v^2) and on the mass surface density
+        // B / <L/M> -- the numerators of eqs. 14, 15 and 19 before the division by B_tot: no square root, one reciprocal
+        const T sc = BULGE ? T(1) : fast_exp2(shift);
+        const T Bv = cosphi * vc * kB;
+        oB = Btot * sc;
+        oV = Bv * sc;
+        oS = fma(Bv * Bv, invB, fma(vc * vc, qB, IbL)) * sc;
+        oLM = Stot * sc;
+    } else {
+        oV = cosphi * vc * kB * invB;
+        oS = fast_sqrt(fma(vc * vc, qB, IbL) * invB);
+        oLM = Btot * fast_rcp(Stot);
+        oB = BULGE ? Btot : Btot * fast_exp2(shift);
     }
 }
 
@@ -804,7 +828,7 @@ constexpr int lbc_blocks(int lbc, int P, bool f64) {
 // the rotation and the store address are shared by S cells and S independent dependency chains are in flight.
 // dst[(row * 4 + observable) * NFB + x].  GUARD: some of the S rows lie past the grid (zero-weight tap padding): they
 // are written as zeros.
-template <typename T, int S, int NFB, int GRP, int PADV, bool BULGE, int SHIFT, bool GUARD>
+template <typename T, int S, int NFB, int GRP, int PADV, bool BULGE, int SHIFT, bool GUARD, bool FLUX>
 BANG_D void eval_superrow(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs, const T* __restrict__ vtab, T* __restrict__ dst,
                           const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
     const T b0 = (T)(jy0 - k.jcy);
@@ -821,20 +845,20 @@ BANG_D void eval_superrow(const CellK<T>& k, const T* __restrict__ bbase, const 
                 vB = vV = vS = vL = T(0);
             } else {
                 const T xp = j == 0 ? px : fma((T)j, k.hs, px), yp = j == 0 ? py : fma((T)j, k.hc, py);
-                eval_cell<T, BULGE, SHIFT>(k, bbase, bs, vtab, xp, yp, vB, vV, vS, vL);
+                eval_cell<T, BULGE, SHIFT, FLUX>(k, bbase, bs, vtab, xp, yp, vB, vV, vS, vL);
             }
             d[(j * 4 + 0) * NFB] = vB; d[(j * 4 + 1) * NFB] = vV; d[(j * 4 + 2) * NFB] = vS; d[(j * 4 + 3) * NFB] = vL;
         }
     }
 }
-template <typename T, int S, int NFB, int GRP, int PADV, bool GUARD>
+template <typename T, int S, int NFB, int GRP, int PADV, bool GUARD, bool FLUX>
 BANG_D void eval_superrow_any(const unsigned comps, const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs, const T* __restrict__ vtab,
                               T* __restrict__ dst, const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
-    if (comps & C_BULGE) eval_superrow<T, S, NFB, GRP, PADV, true, 0, GUARD>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+    if (comps & C_BULGE) eval_superrow<T, S, NFB, GRP, PADV, true, 0, GUARD, FLUX>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_superrow<T, S, NFB, GRP, PADV, false, 3, GUARD>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else if (comps & C_DISC1) eval_superrow<T, S, NFB, GRP, PADV, false, 1, GUARD>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else eval_superrow<T, S, NFB, GRP, PADV, false, 2, GUARD>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+        eval_superrow<T, S, NFB, GRP, PADV, false, 3, GUARD, FLUX>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else if (comps & C_DISC1) eval_superrow<T, S, NFB, GRP, PADV, false, 1, GUARD, FLUX>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else eval_superrow<T, S, NFB, GRP, PADV, false, 2, GUARD, FLUX>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
 }
 
 // ---- the fused kernel ---------------------------------------------------------------------------------------------
@@ -863,7 +887,7 @@ inline size_t vtab_bytes() { return ((size_t)kVcOct * (1 << TabCfg<T>::M) + 1) *
 // scratch for the nodes of Itilde_ext: the row buffer serves when there is one (k_fused), else (k_fine) it is allocated
 template <typename T>
 inline size_t ext_scratch_elems(const GridC& g) {
-    return has_ext(g) ? ((size_t)kBOct * (1 << TabCfg<T>::M)) * (TabCfg<T>::D + 1) + 4 : 0;
+    return has_ext(g) ? ((size_t)kBOct * (1 << TabCfg<T>::M)) * (TabCfg<T>::D + 1) + 4 + (size_t)kBOct * kExtMaxND + 4 : 0;
 }
 template <typename T>
 inline size_t fused_smem_bytes(const GridC& g, int S, int nfb) {
@@ -911,8 +935,14 @@ BANG_D void load_run(const T* __restrict__ src, T (&f)[N]) {
 BANG_D float inv_ml(float x) { return fast_rcp(fmaxf(x, 1e-30f)); }
 BANG_D double inv_ml(double x) { return 1.0 / fmax(x, 1e-300); }
 
-// MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike)
-template <typename T, int S, int NACC, int P, int MODE, int LBC>
+// MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike).
+// FLUX: the flux-weighted PSF of reading G' -- the four fields that go through the PSF and the rebin are the light moments
+// B, B v, B (sigma^2 + v^2) and the mass surface density (eval_cell<FLUX>); the observables are formed per data pixel when
+// its row completes: v = M1/M0, sigma^2 = M2/M0 - v^2, M/L = M3/M0.  The four moments of a pixel are then needed
+// together, so in this instantiation the PSF threads are numbered observable-fastest (lane = 4 group + observable) and the
+// moments travel by warp shuffle inside each quad of lanes; the paper's path (FLUX = false) keeps its own numbering and
+// carries none of this code.
+template <typename T, int S, int NACC, int P, int MODE, int LBC, bool FLUX = false>
 __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T) == 8)) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     constexpr int RUN = (P - 1 + NACC) * S;          // fine cells one thread reads per row for its P data pixels
@@ -934,7 +964,8 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
     const int G = p.nxp / P;                         // pixel groups per map
     constexpr int GMAX = lbc_threads(LBC) / 4;       // pitch of the data array's pixel-group axis (compile-time: immediate offsets)
     const int items = 4 * G;
-    const int q = tid / G, grp = tid - q * G;        // this thread's observable and pixel group in the PSF phase
+    // this thread's observable and pixel group in the PSF phase
+    const int q = FLUX ? (tid & 3) : tid / G, grp = FLUX ? (tid >> 2) : tid - q * G;
     const bool psf_thread = tid < items;
     const int nsuper = g.ny + NACC - 1;
     const size_t npix = (size_t)g.nx * g.ny;
@@ -982,8 +1013,8 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
             // the per-theta constants are re-read from shared memory for every super-row (a handful of broadcast loads)
             // so that they do not occupy registers during the PSF phase
             const CellK<T> k = load_cellk<T>(c);
-            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, GRP, PADV, false>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
-            else eval_superrow_any<T, S, nfb, GRP, PADV, true>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, GRP, PADV, false, FLUX>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            else eval_superrow_any<T, S, nfb, GRP, PADV, true, FLUX>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
             vt = vt + 32 < NT ? vt + 32 : vt + 32 - NT;      // rotate the column ownership by one warp: the ragged last
                                                              // pass then falls on a different warp (scheduler) each time
             __syncthreads();
@@ -1015,11 +1046,24 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
                 }
                 // ---- a6 (or map output): data row py is complete
                 if (py >= 0) {
+                    [[maybe_unused]] unsigned quad_mask = 0;
+                    if constexpr (FLUX) quad_mask = __activemask();        // whole quads: the PSF threads are a multiple of 4
 #pragma unroll
                     for (int i = 0; i < P; ++i) {
                         const int px = grp * P + i;
                         T m = acc[i][0];
-                        if (q == 3) m = inv_ml(m);                     // M/L = 1/<L/M> (fn 10)
+                        if constexpr (FLUX) {
+                            // reading G': B = M0, v = M1/M0, sigma^2 = M2/M0 - v^2, M/L = M3/M0 (M0 floored far below any
+                            // physical light so that padded pixels stay finite)
+                            const int base = (tid & 31) & ~3;
+                            const T m0 = __shfl_sync(quad_mask, m, base), m1 = __shfl_sync(quad_mask, m, base + 1);
+                            const T i0 = inv_ml(m0), v = m1 * i0;
+                            if (q == 1) m = v;
+                            else if (q == 2) m = fast_sqrt(fmax(fma(m, i0, -v * v), T(0)));
+                            else if (q == 3) m = m * i0;
+                        } else {
+                            if (q == 3) m = inv_ml(m);                 // M/L = 1/<L/M> (fn 10)
+                        }
                         if constexpr (MODE == 0) {
                             if (px < g.nx) p.maps[((size_t)b * 4 + q) * npix + (size_t)py * g.nx + px] = m;
                         } else {

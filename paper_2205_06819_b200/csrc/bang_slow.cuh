@@ -59,10 +59,13 @@ __global__ void __launch_bounds__(256) k_slow(const __grid_constant__ SlowParams
         const int nrows = (g.ny + NACC - 1) * S;
         for (int jy = 0; jy < nrows; ++jy) {
             const int sr = jy / S, j = jy - sr * S;
-            // a2 + a3: one fine row, directly
+            // a2 + a3: one fine row, directly (reading G': the light moments)
             for (int x = tid; x < nfx; x += NT) {
                 T o[4] = {T(0), T(0), T(0), T(0)};
-                if (jy < g.nfy) eval_cell_direct<T, false>(c, g, p.btab, p.Ftab, p.direct, x - k.jcx, jy - k.jcy, o);
+                if (jy < g.nfy) {
+                    if (g.flux) eval_cell_direct<T, true>(c, g, p.btab, p.Ftab, p.direct, x - k.jcx, jy - k.jcy, o);
+                    else eval_cell_direct<T, false>(c, g, p.btab, p.Ftab, p.direct, x - k.jcx, jy - k.jcy, o);
+                }
 #pragma unroll
                 for (int q = 0; q < 4; ++q) fine[q * nfx + x] = o[q];
             }
@@ -79,12 +82,22 @@ __global__ void __launch_bounds__(256) k_slow(const __grid_constant__ SlowParams
                         a = fma((T)p.W[(NACC - 1 - kk) * S + j], xs, a);
                     }
                 }
-                const int py0 = sr - (NACC - 1);
-                if (j == S - 1 && py0 >= 0) {                        // a6 (or map output): data row py0 is complete
-                    T& a = acc[((py0 % NACC) * 4 + q) * nx + px];
-                    T m = a;
-                    a = T(0);
-                    if (q == 3) m = inv_ml(m);
+            }
+            __syncthreads();
+            const int py0 = sr - (NACC - 1);
+            if (j == S - 1 && py0 >= 0) {                            // a6 (or map output): data row py0 is complete
+                T* row = acc + (size_t)(py0 % NACC) * 4 * nx;
+                for (int item = tid; item < 4 * nx; item += NT) {
+                    const int q = item / nx, px = item - q * nx;
+                    T m = row[q * nx + px];
+                    if (g.flux) {                                    // reading G': v = M1/M0, sigma^2 = M2/M0 - v^2, M/L = M3/M0
+                        const T i0 = inv_ml(row[px]), v = row[nx + px] * i0;
+                        if (q == 1) m = v;
+                        else if (q == 2) m = fast_sqrt(fmax(fma(m, i0, -v * v), T(0)));
+                        else if (q == 3) m = m * i0;
+                    } else if (q == 3) {
+                        m = inv_ml(m);
+                    }
                     if constexpr (MODE == 0) {
                         p.maps[((size_t)b * 4 + q) * npix + (size_t)py0 * nx + px] = m;
                     } else {
@@ -94,8 +107,10 @@ __global__ void __launch_bounds__(256) k_slow(const __grid_constant__ SlowParams
                         chi2 = de.y != 0.0 ? fma(z, z, chi2) : chi2;
                     }
                 }
+                __syncthreads();
+                for (int item = tid; item < 4 * nx; item += NT) row[item] = T(0);
+                __syncthreads();
             }
-            __syncthreads();
         }
         if constexpr (MODE == 1) {
 #pragma unroll
