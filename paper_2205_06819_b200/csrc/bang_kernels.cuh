@@ -76,6 +76,7 @@ struct ThetaC {
     T cexp[2], ampBd[2], ampSd[2]; // disc j: B_d = ampBd 2^(r cexp), Sigma_d = ampSd 2^(r cexp) = (M/L)_d B_d
     T vkB[2], q3B[2];            // -sin i k_j ampBd_j   and   (1 - k_j^2)/3 ampBd_j: the light weights of eqs. 14, 15
     ThetaD d;
+    alignas(16) int kpack[28];   // fp32 mode: the CellK constants below, packed for 128-bit broadcast loads (pack_cellk)
 };
 
 // geometry of the run, the same for every theta (built on the host at bang_create)
@@ -319,6 +320,7 @@ BANG_D void decode_theta(const double* __restrict__ th, const GridC& g, const Po
     c.vc_near = (T)sqrt(vc2_total<T>(d, g, g.comps, Ftab, sqrt(R2min + yp0 * yp0 * tan2i)));
     c.valid = 1;
 }
+template <typename T> BANG_D void pack_cellk(ThetaC<T>& c);
 
 // Node values -> monomial coefficients, in place: cells x (D+1) values at the Chebyshev nodes of each interval become the
 // D+1 coefficients of its interpolant (fit.vinv, fp64 arithmetic).  One thread per interval; no barrier inside.
@@ -534,13 +536,39 @@ struct CellK {
 template <typename T>
 BANG_D CellK<T> load_cellk(const ThetaC<T>& c) {
     CellK<T> k;
-    k.jcx = c.jcx; k.jcy = c.jcy; k.vfirst1 = c.vfirst - 1; k.vlast = c.vcells;
-    k.bfirst1 = c.bfirst - 1; k.blast = c.bcells;
-    k.hc = c.hc; k.hs = c.hs; k.xp0 = c.xp0; k.yp0 = c.yp0; k.tan2i = c.tan2i;
-    k.invRb2 = c.invRb2; k.ampBb = c.ampBb; k.ampIb = c.ampIb; k.MLb = c.MLb;
-    k.cexp0 = c.cexp[0]; k.cexp1 = c.cexp[1]; k.ampBd0 = c.ampBd[0]; k.ampBd1 = c.ampBd[1];
-    k.ampSd0 = c.ampSd[0]; k.ampSd1 = c.ampSd[1]; k.vkB0 = c.vkB[0]; k.vkB1 = c.vkB[1]; k.q3B0 = c.q3B[0]; k.q3B1 = c.q3B[1];
+    if constexpr (sizeof(T) == 4) {
+        // seven 128-bit broadcast loads instead of 25 scalar ones: the constants are re-read every super-row, and a
+        // broadcast load costs a wavefront of the shared-memory pipe whatever its width
+        const int4* s = reinterpret_cast<const int4*>(c.kpack);
+        const int4 a = s[0], b = s[1], e = s[2], f = s[3], g = s[4], h = s[5];
+        k.jcx = a.x; k.jcy = a.y; k.vfirst1 = a.z; k.bfirst1 = a.w;
+        k.hc = __int_as_float(b.x); k.hs = __int_as_float(b.y); k.xp0 = __int_as_float(b.z); k.yp0 = __int_as_float(b.w);
+        k.tan2i = __int_as_float(e.x); k.invRb2 = __int_as_float(e.y); k.ampBb = __int_as_float(e.z); k.ampIb = __int_as_float(e.w);
+        k.MLb = __int_as_float(f.x); k.cexp0 = __int_as_float(f.y); k.cexp1 = __int_as_float(f.z); k.ampBd0 = __int_as_float(f.w);
+        k.ampBd1 = __int_as_float(g.x); k.ampSd0 = __int_as_float(g.y); k.ampSd1 = __int_as_float(g.z); k.vkB0 = __int_as_float(g.w);
+        k.vkB1 = __int_as_float(h.x); k.q3B0 = __int_as_float(h.y); k.q3B1 = __int_as_float(h.z);
+        k.vlast = c.vcells; k.blast = c.bcells;      // read only by BANG_CHECK builds
+    } else {
+        k.jcx = c.jcx; k.jcy = c.jcy; k.vfirst1 = c.vfirst - 1; k.vlast = c.vcells;
+        k.bfirst1 = c.bfirst - 1; k.blast = c.bcells;
+        k.hc = c.hc; k.hs = c.hs; k.xp0 = c.xp0; k.yp0 = c.yp0; k.tan2i = c.tan2i;
+        k.invRb2 = c.invRb2; k.ampBb = c.ampBb; k.ampIb = c.ampIb; k.MLb = c.MLb;
+        k.cexp0 = c.cexp[0]; k.cexp1 = c.cexp[1]; k.ampBd0 = c.ampBd[0]; k.ampBd1 = c.ampBd[1];
+        k.ampSd0 = c.ampSd[0]; k.ampSd1 = c.ampSd[1]; k.vkB0 = c.vkB[0]; k.vkB1 = c.vkB[1]; k.q3B0 = c.q3B[0]; k.q3B1 = c.q3B[1];
+    }
     return k;
+}
+// fills ThetaC::kpack from the decoded fields (the thread that ran decode_theta; fp32 mode only)
+template <typename T>
+BANG_D void pack_cellk(ThetaC<T>& c) {
+    if constexpr (sizeof(T) == 4) {
+        int* q = c.kpack;
+        q[0] = c.jcx; q[1] = c.jcy; q[2] = c.vfirst - 1; q[3] = c.bfirst - 1;
+        const float v[19] = {c.hc, c.hs, c.xp0, c.yp0, c.tan2i, c.invRb2, c.ampBb, c.ampIb, c.MLb, c.cexp[0], c.cexp[1],
+                             c.ampBd[0], c.ampBd[1], c.ampSd[0], c.ampSd[1], c.vkB[0], c.vkB[1], c.q3B[0], c.q3B[1]};
+#pragma unroll
+        for (int i = 0; i < 19; ++i) q[4 + i] = __float_as_int(v[i]);
+    }
 }
 
 // sec. 2.1: rotate into the galaxy frame (fn 2).  a = jx - jcx and b = jy - jcy are offsets in cells from
@@ -976,7 +1004,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
 
     for (int b = blockIdx.x; b < p.B; b += gridDim.x) {
         __syncthreads();
-        if (tid == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.btab, p.Ftab, c);
+        if (tid == 0) { decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.btab, p.Ftab, c); pack_cellk<T>(c); }
         __syncthreads();
         if (!c.valid || (c.slow && !p.slow_list)) {  // out-of-domain theta: NaN maps / -inf likelihood
             if constexpr (MODE == 0) {
@@ -1123,7 +1151,7 @@ __global__ void __launch_bounds__(256) k_fine(const __grid_constant__ FineParams
     const T* bbase = p.btab.coef - (ptrdiff_t)p.btab.first * (2 * NC);
     for (int b = blockIdx.x; b < p.B; b += gridDim.x) {
         __syncthreads();
-        if (threadIdx.x == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.btab, p.Ftab, c);
+        if (threadIdx.x == 0) { decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.btab, p.Ftab, c); pack_cellk<T>(c); }
         __syncthreads();
         T* out = p.fine + (size_t)b * 4 * plane;
         if (!c.valid) {

@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(256) k_slow(const __grid_constant__ SlowParams
     for (int li = blockIdx.x; li < n; li += gridDim.x) {
         const int b = p.slow_list[li];
         __syncthreads();
-        if (tid == 0) decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.btab, p.Ftab, c);
+        if (tid == 0) { decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.btab, p.Ftab, c); pack_cellk<T>(c); }
         for (int i = tid; i < NACC * 4 * nx; i += NT) acc[i] = T(0);
         __syncthreads();
         const CellK<T> k = load_cellk<T>(c);
