@@ -21,6 +21,7 @@ struct bang_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
     int n_sm = 0;
+    int smem_optin = 0;                    // cudaDevAttrMaxSharedMemoryPerBlockOptin: every kernel is opted in to this maximum
     GridC g{};
     FitC fit{};
     int rk = 0, nacc = 0, P = 0, nxp = 0, threads = 0;
@@ -28,7 +29,7 @@ struct bang_ctx {
     void* btab = nullptr; int btab_first = 0, btab_cells = 0;
     void* Ftab = nullptr; int Ftab_first = 0, Ftab_cells = 0;
     double2* data = nullptr; double C0 = 0.0; bool has_data = false;
-    double* scal = nullptr;                // device scratch: {C0, bad-pixel count}
+    double* scal = nullptr;                // device scratch: {C0, bad-pixel count}, per-CTA partial sums, the ticket counter
     double* gl_dev = nullptr;              // N_J Gauss-Legendre nodes then weights (reading B): table build, direct path
     double2* qd_dev = nullptr; float2* qf_dev = nullptr;   // the same rule as {a_k, b_k} pairs (reading U', ext_Itilde)
     // staging for the *_host calls
@@ -41,6 +42,7 @@ struct bang_ctx {
     // is too large for k_slow's shared memory (such theta are then reported as out of domain)
     int* slow_list = nullptr; int* slow_cnt = nullptr; int slow_cap = 0; size_t slow_smem = 0;
     double* W_dev = nullptr;               // composite taps on the device (direct path)
+    bool fine_ready = false;               // k_fine's shared-memory opt-in done (once per context)
     // bang_ns_walk scratch: proposals [K][d], their theta [K][17] and likelihoods [K], Cholesky factors + scales, counts
     double* ns_prop = nullptr; double* ns_theta = nullptr; double* ns_pl = nullptr; double* ns_chol = nullptr;
     int* ns_acc = nullptr; int ns_capK = 0, ns_capG = 0;
@@ -171,13 +173,17 @@ __global__ void k_univ_fit(int n_rows, FitC fit, const double* __restrict__ vals
 
 // data preparation (layout [ny][4][P][gmax], gmax >= nxp/P the pixel-group pitch of the launch's thread class; the
 // caller zeroes the buffer): {d, 1/e} per used pixel ({0,0} where masked or padded), C0 = sum -1/2 ln(2 pi e^2), and the number
-// of used pixels with err <= 0 or a non-finite value.  One block, deterministic reduction order.
-__global__ void k_prep_data(int nx, int ny, int nxp, int P, int gmax, const double* __restrict__ data, const double* __restrict__ err,
-                            const unsigned char* __restrict__ mask, double2* __restrict__ out, double* __restrict__ scal) {
-    __shared__ double sh[2][32];
+// of used pixels with err <= 0 or a non-finite value.  A grid of CTAs; per-CTA partial sums go to scal[2 + 2 blk ..] and the
+// last CTA to finish adds them in CTA order: the reduction order is fixed, the result deterministic.
+constexpr int kPrepMaxBlocks = 64;
+__global__ void __launch_bounds__(256) k_prep_data(int nx, int ny, int nxp, int P, int gmax, const double* __restrict__ data,
+                                                   const double* __restrict__ err, const unsigned char* __restrict__ mask,
+                                                   double2* __restrict__ out, double* __restrict__ scal, unsigned* __restrict__ ticket) {
+    __shared__ double sh[2][8];
+    __shared__ bool last;
     double c0 = 0.0, bad = 0.0;
     const int total = ny * 4 * nxp;
-    for (int i = threadIdx.x; i < total; i += blockDim.x) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
         const int px = i % nxp, q = (i / nxp) % 4, py = i / (4 * nxp);
         double2 v = make_double2(0.0, 0.0);
         if (px < nx) {
@@ -203,7 +209,17 @@ __global__ void k_prep_data(int nx, int ny, int nxp, int P, int gmax, const doub
     if (threadIdx.x == 0) {
         double a = 0.0, b = 0.0;
         for (int w = 0; w < (int)(blockDim.x + 31) / 32; ++w) { a += sh[0][w]; b += sh[1][w]; }
+        scal[2 + 2 * blockIdx.x] = a; scal[3 + 2 * blockIdx.x] = b;
+        __threadfence();
+        last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (last && threadIdx.x == 0) {
+        __threadfence();
+        double a = 0.0, b = 0.0;
+        for (unsigned k = 0; k < gridDim.x; ++k) { a += scal[2 + 2 * k]; b += scal[3 + 2 * k]; }
         scal[0] = a; scal[1] = b;
+        *ticket = 0u;
     }
 }
 
@@ -310,7 +326,7 @@ FusedLaunch make_launch(bang_ctx* c, const double* theta, int B, int mode, void*
     L.W = c->W.data(); L.nacc = c->nacc;
     L.theta = theta; L.B = B; L.P = c->P; L.nxp = c->nxp; L.mode = mode;
     L.maps = maps; L.data = c->data; L.C0 = c->C0; L.logL = logL;
-    L.threads = c->threads; L.ctas = c->force_ctas; L.n_sm = c->n_sm; L.stream = c->stream;
+    L.threads = c->threads; L.ctas = c->force_ctas; L.n_sm = c->n_sm; L.smem_optin = c->smem_optin; L.stream = c->stream;
     L.cache = c->launch_cache;
     L.slow_list = c->slow_smem ? c->slow_list : nullptr; L.slow_count = c->slow_cnt;
     return L;
@@ -354,8 +370,10 @@ int setup_slow(bang_ctx* ctx) {
     cudaDeviceProp prop;
     CU(cudaGetDeviceProperties(&prop, ctx->device));
     if (smem > prop.sharedMemPerBlockOptin) return BANG_OK;          // slow_smem stays 0: no direct path on this grid
-    CU(cudaFuncSetAttribute(k_slow<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CU(cudaFuncSetAttribute(k_slow<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // opted in to the device maximum, not to this context's size: the attribute is per function, and another context
+    // of the same instantiation may need more
+    CU(cudaFuncSetAttribute(k_slow<T, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
+    CU(cudaFuncSetAttribute(k_slow<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin));
     CU(cudaMalloc(&ctx->slow_cnt, 2 * sizeof(int)));
     CU(cudaMemsetAsync(ctx->slow_cnt, 0, 2 * sizeof(int), ctx->stream));
     ctx->slow_smem = smem;
@@ -508,6 +526,7 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete ctx; return BANG_ECUDA; }
     ctx->n_sm = prop.multiProcessorCount;
+    ctx->smem_optin = (int)prop.sharedMemPerBlockOptin;
 
     const bool f64 = model->precision == BANG_FP64;
     ctx->rk = rk; ctx->nacc = nacc;
@@ -552,7 +571,7 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
     const int items = 4 * ctx->nxp / P;
     ctx->threads = std::max(128, (items + 31) / 32 * 32);
 #ifdef BANG_TUNING
-    if (const char* e = getenv("BANG_THREADS")) if (atoi(e) >= ctx->threads && atoi(e) <= 512) ctx->threads = atoi(e) / 32 * 32;
+    if (const char* e = getenv("BANG_THREADS")) if (atoi(e) >= (items + 31) / 32 * 32 && atoi(e) <= 512) ctx->threads = atoi(e) / 32 * 32;
     if (const char* e = getenv("BANG_CTAS")) if (atoi(e) > 0) ctx->force_ctas = atoi(e);
 #endif
     if (ctx->threads > 512) { delete ctx; return BANG_EINVAL; }      // row too wide for one CTA
@@ -586,7 +605,8 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
         rc = f64 ? build_universal<double>(ctx, ctx->gl_dev, ctx->gl_dev + model->jeans_nodes)
                  : build_universal<float>(ctx, ctx->gl_dev, ctx->gl_dev + model->jeans_nodes);
         if (rc != BANG_OK) break;
-        if (cudaMalloc(&ctx->scal, 2 * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
+        if (cudaMalloc(&ctx->scal, (4 + 2 * kPrepMaxBlocks) * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
+        if (cudaMemsetAsync(ctx->scal, 0, (4 + 2 * kPrepMaxBlocks) * sizeof(double), ctx->stream) != cudaSuccess) { rc = BANG_ECUDA; break; }
         if (cudaMalloc(&ctx->W_dev, ctx->W.size() * sizeof(double)) != cudaSuccess) { rc = BANG_ENOMEM; break; }
         if (cudaMemcpyAsync(ctx->W_dev, ctx->W.data(), ctx->W.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream) != cudaSuccess ||
             cudaStreamSynchronize(ctx->stream) != cudaSuccess) { rc = BANG_ECUDA; break; }
@@ -612,7 +632,10 @@ int bang_set_data(bang_ctx* ctx, const double* data_dev, const double* err_dev, 
     const size_t n = (size_t)ctx->g.ny * 4 * ctx->P * gmax;
     CU(cudaMalloc(&buf, n * sizeof(double2)));
     CU(cudaMemsetAsync(buf, 0, n * sizeof(double2), ctx->stream));
-    k_prep_data<<<1, 1024, 0, ctx->stream>>>(ctx->g.nx, ctx->g.ny, ctx->nxp, ctx->P, gmax, data_dev, err_dev, mask_dev, buf, ctx->scal);
+    const int prep_total = ctx->g.ny * 4 * ctx->nxp;
+    const int prep_blocks = std::max(1, std::min(kPrepMaxBlocks, (prep_total + 1023) / 1024));
+    k_prep_data<<<prep_blocks, 256, 0, ctx->stream>>>(ctx->g.nx, ctx->g.ny, ctx->nxp, ctx->P, gmax, data_dev, err_dev, mask_dev, buf, ctx->scal,
+                                                    reinterpret_cast<unsigned*>(ctx->scal + 2 + 2 * kPrepMaxBlocks));
     ctx->launches += 1;
     double scal[2] = {0, 0};
     cudaError_t e = cudaGetLastError();
@@ -731,7 +754,7 @@ int bang_model_fine(bang_ctx* ctx, const double* theta_dev, int B, void* fine_de
                              PolyTab<double>{static_cast<const double*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells},
                              direct, (int)bs_elems<double>(ctx->g), theta_dev, B, static_cast<double*>(fine_dev)};
         const size_t smem = fused_smem_bytes<double>(ctx->g, 0, 0);
-        CU(cudaFuncSetAttribute(k_fine<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (!ctx->fine_ready) CU(cudaFuncSetAttribute(k_fine<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin));
         k_fine<double><<<ctas, 256, smem, ctx->stream>>>(p);
     } else {
         FineParams<float> p{ctx->g, ctx->fit,
@@ -739,11 +762,12 @@ int bang_model_fine(bang_ctx* ctx, const double* theta_dev, int B, void* fine_de
                             PolyTab<float>{static_cast<const float*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells},
                             direct, (int)bs_elems<float>(ctx->g), theta_dev, B, static_cast<float*>(fine_dev)};
         const size_t smem = fused_smem_bytes<float>(ctx->g, 0, 0);
-        CU(cudaFuncSetAttribute(k_fine<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (!ctx->fine_ready) CU(cudaFuncSetAttribute(k_fine<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem_optin));
         k_fine<float><<<ctas, 256, smem, ctx->stream>>>(p);
     }
     ctx->launches += 1;
     CU(cudaGetLastError());
+    ctx->fine_ready = true;
     return BANG_OK;
 }
 

@@ -23,7 +23,10 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     int per_sm = L.cache ? L.cache[L.mode] : 0;
     cudaError_t e;
     if (per_sm < 1) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (smem > (size_t)L.smem_optin) return cudaErrorLaunchOutOfResources;
+        // opted in to the device maximum, not to this launch's size: the attribute is per function, and another context
+        // of the same instantiation (reading U' in fp64 mode) may need more
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L.smem_optin);
         if (e != cudaSuccess) return e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, L.threads, smem);
         if (e != cudaSuccess) return e;

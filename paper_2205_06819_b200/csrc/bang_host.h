@@ -23,6 +23,7 @@ struct FusedLaunch {
     int* slow_list; int* slow_count;   // theta left to the direct path (k_slow), see FusedParams
     int threads, ctas;           // launch shape (ctas = 0: let the launcher size a persistent grid)
     int n_sm;
+    int smem_optin;              // the device's opt-in maximum of dynamic shared memory per CTA
     int* cache;                  // [2] resident CTAs per SM of the mode's kernel once configured (0 = not yet), or NULL
     cudaStream_t stream;
 };

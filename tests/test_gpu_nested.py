@@ -112,3 +112,64 @@ def test_device_nested_sampling_orders_the_config4_variants(oracle):
         ctx.close()
     assert logz["B+2D+H"] > max(logz[v] for v in ("B+D", "B+2D", "2D+H")) + 10.0, logz     # eq. 17: ln B >> 0
     assert logz["B+D"] < min(logz[v] for v in ("B+2D", "B+2D+H")) - 100.0, logz
+
+
+# ------------------------------------------------------------------------------------------------ the device walker, pinned
+def _philox4x32_10(c0, c1, c2, c3, k0, k1):
+    """Philox4x32-10 (Salmon et al. 2011) restated with numpy uint64 arithmetic; arrays of counters, scalar key."""
+    M0, M1, W0, W1 = np.uint64(0xD2511F53), np.uint64(0xCD9E8D57), 0x9E3779B9, 0xBB67AE85
+    mask = np.uint64(0xFFFFFFFF)
+    c = [np.asarray(x, dtype=np.uint64) for x in (c0, c1, c2, c3)]
+    for r in range(10):
+        p0, p1 = M0 * c[0], M1 * c[2]
+        kk0, kk1 = np.uint64((k0 + r * W0) & 0xFFFFFFFF), np.uint64((k1 + r * W1) & 0xFFFFFFFF)
+        c = [((p1 >> np.uint64(32)) ^ c[1] ^ kk0) & mask, p1 & mask, ((p0 >> np.uint64(32)) ^ c[3] ^ kk1) & mask, p0 & mask]
+    return c
+
+
+def test_ns_walk_proposals_follow_the_documented_generator(oracle):
+    # one step with no likelihood bound: every proposal that stays in the cube is accepted, so the walkers end AT their
+    # proposals u + scale (2.38/sqrt d) chol z, z from Philox4x32-10 (counter = (walker, step, draw), key = seed) and
+    # Box-Muller, as include/bang.h states -- restated here in numpy.  Their logL is the kernel's own.
+    import torch
+    from paper_2205_06819_b200 import bang
+    cfg = W.config(1)
+    tt = W.theta_true(1)
+    data, err, mask = W.make_data(1, oracle.model_maps(tt, cfg)[0])
+    ctx = bang.Context(cfg, precision="fp64")
+    ctx.set_data(data, err, mask)
+    K, d, seed = 200, 5, 0x1234567890ABCDEF
+    free = [2, 3, 4, 6, 13]
+    lo, hi = tt[free] * 0.9, tt[free] * 1.1
+    rng = np.random.default_rng(3)
+    u0 = 0.3 + 0.4 * rng.random((K, d))
+    A = rng.normal(size=(2, d, d)) * 0.02
+    chol = np.stack([np.linalg.cholesky(a @ a.T + 1e-4 * np.eye(d)) for a in A])
+    scale = np.array([1.0, 0.5])
+    group = (np.arange(K) % 2).astype(np.int32)
+    u = torch.as_tensor(u0.copy(), device="cuda")
+    ll = torch.full((K,), -np.inf, dtype=torch.float64, device="cuda")
+    lstar = torch.full((K,), -np.inf, dtype=torch.float64, device="cuda")
+    n_acc = ctx.ns_walk(u, ll, lstar, torch.as_tensor(group, device="cuda"), chol, scale, free, lo, hi, tt, steps=1, seed=seed)
+    k = np.arange(K)
+    z = np.zeros((K, 8))
+    for blk in range(2):
+        r = _philox4x32_10(k, np.zeros(K), np.full(K, blk), np.zeros(K), seed & 0xFFFFFFFF, seed >> 32)
+        for h in range(2):
+            u1 = (r[2 * h].astype(np.float64) + 1.0) / 4294967296.0
+            u2 = r[2 * h + 1].astype(np.float64) / 4294967296.0
+            rad = np.sqrt(-2.0 * np.log(u1))
+            z[:, 4 * blk + 2 * h] = rad * np.cos(2 * np.pi * u2)
+            z[:, 4 * blk + 2 * h + 1] = rad * np.sin(2 * np.pi * u2)
+    want = u0 + (scale[group] * 2.38 / np.sqrt(d))[:, None] * np.einsum("kij,kj->ki", chol[group], z[:, :d])
+    inside = np.all((want >= 0) & (want <= 1), axis=1)
+    assert inside.sum() > K // 2
+    got = u.cpu().numpy()
+    assert np.allclose(got[inside], want[inside], rtol=0, atol=1e-13)
+    assert np.array_equal(got[~inside], u0[~inside])                     # outside the cube: theta = NaN, logL = -inf, rejected
+    assert n_acc.sum() == inside.sum() and n_acc[0] == inside[group == 0].sum()
+    th = np.repeat(tt[None], K, axis=0)
+    th[:, free] = lo + (hi - lo) * got
+    # (theta is rebuilt here without the kernel's fused multiply-add: equal to rounding, not bit for bit)
+    assert np.allclose(ll.cpu().numpy()[inside], ctx.loglike_host(th)[inside], rtol=1e-9, atol=0)
+    ctx.close()

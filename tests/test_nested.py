@@ -72,3 +72,25 @@ def test_box_transform_and_out_of_domain_points():
     f = lambda u: np.where(u[:, 0] < 0.5, -np.inf, g(u))
     r = NestedSampler(f, 2, nlive=400, batch=40, mcmc_steps=25, seed=21).run()
     assert abs(r.logZ) < 3 * r.logZ_err + 0.05
+
+
+def test_philox_restatement_against_the_published_known_answers():
+    # the numpy restatement of Philox4x32-10 that tests/test_gpu_nested.py uses to check bang_ns_walk's proposals,
+    # against Random123's known-answer vectors for philox4x32-10 (Salmon et al. 2011)
+    from test_gpu_nested import _philox4x32_10
+    out = _philox4x32_10([0], [0], [0], [0], 0, 0)
+    assert [int(x[0]) for x in out] == [0x6627E8D5, 0xE169C58D, 0xBC57AC4C, 0x9B00DBD8]
+    out = _philox4x32_10([0xFFFFFFFF], [0xFFFFFFFF], [0xFFFFFFFF], [0xFFFFFFFF], 0xFFFFFFFF, 0xFFFFFFFF)
+    assert [int(x[0]) for x in out] == [0x408F276D, 0x41C83B0E, 0xA20BC7C6, 0x6D5451FD]
+    out = _philox4x32_10([0x243F6A88], [0x85A308D3], [0x13198A2E], [0x03707344], 0xA4093822, 0x299F31D0)
+    assert [int(x[0]) for x in out] == [0xD16CFE09, 0x94FDCCEB, 0x5001E420, 0x24126EA1]
+
+
+def test_combine_runs():
+    from paper_2205_06819_b200.nested import NestedResult, combine_runs
+    mk = lambda z, e: NestedResult(z, e, 1.0, np.zeros((1, 1)), np.zeros(1), np.zeros(1), 1, 1, 0.3)
+    assert combine_runs([mk(-5.0, 0.2)]) == (-5.0, 0.2)
+    lz, err = combine_runs([mk(math.log(1.0), 0.1), mk(math.log(3.0), 0.1)])
+    assert abs(lz - math.log(2.0)) < 1e-12 and abs(err - math.sqrt(2.0) / math.sqrt(2) / 2.0) < 1e-12
+    lz, _ = combine_runs([mk(-1e6 + 1.0, 0.1), mk(-1e6, 0.1)])          # no overflow far from zero
+    assert abs(lz - (-1e6 + math.log((math.e + 1) / 2))) < 1e-9
