@@ -56,7 +56,7 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     p.Ftab = PolyTab<T>{static_cast<const T*>(L.Ftab), L.Ftab_first, L.Ftab_cells};
     p.quad = L.quad; p.bs_elems = (int)bs_elems<T>(L.g);
     for (int t = 0; t < NACC * S; ++t) p.W[t] = (T)L.W[t];
-    p.theta = L.theta; p.B = L.B; p.nxp = L.nxp;
+    p.theta = L.theta; p.B = L.B; p.mode = L.mode; p.nxp = L.nxp;
     p.maps = static_cast<T*>(L.maps); p.data = L.data; p.C0 = L.C0; p.logL = L.logL;
     p.slow_list = L.slow_list; p.slow_count = L.slow_count;
     kern<<<ctas, L.threads, smem, L.stream>>>(p);
@@ -65,17 +65,30 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
 
 template <typename T, int S, int NACC, int P, int LBC>
 cudaError_t launch_lbc(const FusedLaunch& L, FusedInfo* info, bool query_only) {
-    if (L.g.flux)      // reading G': a separate instantiation, so that the paper's path keeps its registers
-        return L.mode == 0 ? launch_mode<T, S, NACC, P, 0, LBC, true>(L, info, query_only)
-                           : launch_mode<T, S, NACC, P, 1, LBC, true>(L, info, query_only);
-    return L.mode == 0 ? launch_mode<T, S, NACC, P, 0, LBC, false>(L, info, query_only)
-                       : launch_mode<T, S, NACC, P, 1, LBC, false>(L, info, query_only);
+    if constexpr (sizeof(T) == 8) {
+        // fp64 mode: one instantiation serves both calls (MODE 2: p.mode read at run time), which halves its build
+        return L.g.flux ? launch_mode<T, S, NACC, P, 2, LBC, true>(L, info, query_only)
+                        : launch_mode<T, S, NACC, P, 2, LBC, false>(L, info, query_only);
+    } else {
+        if (L.g.flux)      // reading G': a separate instantiation, so that the paper's path keeps its registers
+            return L.mode == 0 ? launch_mode<T, S, NACC, P, 0, LBC, true>(L, info, query_only)
+                               : launch_mode<T, S, NACC, P, 1, LBC, true>(L, info, query_only);
+        return L.mode == 0 ? launch_mode<T, S, NACC, P, 0, LBC, false>(L, info, query_only)
+                           : launch_mode<T, S, NACC, P, 1, LBC, false>(L, info, query_only);
+    }
 }
 template <typename T, int S, int NACC, int P>
 cudaError_t launch_one(const FusedLaunch& L, FusedInfo* info, bool query_only) {
     if (L.threads <= 128) return launch_lbc<T, S, NACC, P, 0>(L, info, query_only);
-    if (L.threads <= 256) return launch_lbc<T, S, NACC, P, 1>(L, info, query_only);
-    return launch_lbc<T, S, NACC, P, 2>(L, info, query_only);
+#ifndef BANG_TUNING
+    // fp32 mode takes P = 2 only for maps of up to 64 columns, i.e. 128 threads: the wider classes would be dead code
+    if constexpr (sizeof(T) == 4 && P == 2) return cudaErrorInvalidValue;
+    else
+#endif
+    {
+        if (L.threads <= 256) return launch_lbc<T, S, NACC, P, 1>(L, info, query_only);
+        return launch_lbc<T, S, NACC, P, 2>(L, info, query_only);
+    }
 }
 
 template <typename T, int S, int P>

@@ -900,6 +900,7 @@ struct FusedParams {
     T W[NACC * S];               // composite x s box (*) Gaussian taps, zero padded (a4 + a5)
     const double* theta;         // [B][17]
     int B;
+    int mode;                    // 0 maps, 1 likelihood (read by the MODE = 2 instantiations only)
     int nxp;                     // data columns padded to a multiple of P
     T* maps;                     // [B][4][ny][nx]
     const double2* data;         // [ny][4][P][GMAX] {d, 1/e} of pixel group P + i (1/e = 0 where masked or padded); GMAX =
@@ -963,7 +964,8 @@ BANG_D void load_run(const T* __restrict__ src, T (&f)[N]) {
 BANG_D float inv_ml(float x) { return fast_rcp(fmaxf(x, 1e-30f)); }
 BANG_D double inv_ml(double x) { return 1.0 / fmax(x, 1e-300); }
 
-// MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike).
+// MODE 0: write the maps (bang_model_maps); MODE 1: reduce the likelihood (bang_loglike); MODE 2: either, chosen at run
+// time by p.mode (fp64 mode is instantiated this way only: it halves the build and costs one uniform branch per data row).
 // FLUX: the flux-weighted PSF of reading G' -- the four fields that go through the PSF and the rebin are the light moments
 // B, B v, B (sigma^2 + v^2) and the mass surface density (eval_cell<FLUX>); the observables are formed per data pixel when
 // its row completes: v = M1/M0, sigma^2 = M2/M0 - v^2, M/L = M3/M0.  The four moments of a pixel are then needed
@@ -1007,7 +1009,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
         if (tid == 0) { decode_theta<T>(p.theta + (size_t)b * kNTheta, g, p.btab, p.Ftab, c); pack_cellk<T>(c); }
         __syncthreads();
         if (!c.valid || (c.slow && !p.slow_list)) {  // out-of-domain theta: NaN maps / -inf likelihood
-            if constexpr (MODE == 0) {
+            if (MODE == 0 || (MODE == 2 && p.mode == 0)) {
                 const T qnan = (T)nan("");
                 for (size_t i = tid; i < 4 * npix; i += NT) p.maps[(size_t)b * 4 * npix + i] = qnan;
             } else if (tid == 0) {
@@ -1052,7 +1054,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
                 // a6: this thread's P {d, 1/e} pairs, requested now and used after the taps (the row is padded to nxp,
                 // so the loads need no guard; 1/e = 0 where masked or padded)
                 double2 de[P];
-                if constexpr (MODE == 1) {
+                if (MODE == 1 || (MODE == 2 && p.mode == 1)) {
                     if (py >= 0) {
                         const double2* src = p.data + (((py * 4 + q) * P) * GMAX + grp);
 #pragma unroll
@@ -1092,7 +1094,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
                         } else {
                             if (q == 3) m = inv_ml(m);                 // M/L = 1/<L/M> (fn 10)
                         }
-                        if constexpr (MODE == 0) {
+                        if (MODE == 0 || (MODE == 2 && p.mode == 0)) {
                             if (px < g.nx) p.maps[((size_t)b * 4 + q) * npix + (size_t)py * g.nx + px] = m;
                         } else {
                             const double z = (de[i].x - (double)m) * de[i].y;      // eq. 18, residual in fp64
@@ -1109,7 +1111,7 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
             }
             __syncthreads();
         }
-        if constexpr (MODE == 1) {                   // a6: block reduction, warp shuffles, fp64
+        if (MODE == 1 || (MODE == 2 && p.mode == 1)) {   // a6: block reduction, warp shuffles, fp64
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) chi2 += __shfl_xor_sync(0xffffffffu, chi2, o);
             if ((tid & 31) == 0) red[tid >> 5] = chi2;
