@@ -94,3 +94,64 @@ def test_combine_runs():
     assert abs(lz - math.log(2.0)) < 1e-12 and abs(err - math.sqrt(2.0) / math.sqrt(2) / 2.0) < 1e-12
     lz, _ = combine_runs([mk(-1e6 + 1.0, 0.1), mk(-1e6, 0.1)])          # no overflow far from zero
     assert abs(lz - (-1e6 + math.log((math.e + 1) / 2))) < 1e-9
+
+
+class _StubContext:
+    """A stand-in for bang.Context on the CPU: a Gaussian likelihood in the unit cube and a numpy restatement of what
+    bang_ns_walk does (lock-step constrained Metropolis walks, per-group Cholesky factor and scale, per-walker bound),
+    so that run_device's host side -- several runs in lock-step, retire / replace bookkeeping, evidence -- is tested
+    without a GPU."""
+    device = "cpu"
+
+    def __init__(self, mu, sigma, free, lo, hi):
+        self.mu, self.sigma, self.free, self.lo, self.hi = np.asarray(mu), sigma, list(free), np.asarray(lo), np.asarray(hi)
+        self.calls, self.max_walkers = 0, 0
+
+    def _ll(self, u):
+        d = u.shape[1]
+        return -0.5 * (((u - self.mu) / self.sigma) ** 2).sum(axis=1) - d * math.log(self.sigma * math.sqrt(2 * math.pi))
+
+    def loglike(self, theta):
+        import torch
+        theta = np.asarray(theta)
+        return torch.as_tensor(self._ll((theta[:, self.free] - self.lo) / (self.hi - self.lo)))
+
+    def ns_walk(self, u, logL, Lstar, group, chol, scale, free, lo, hi, theta0, steps, seed=0):
+        rng = np.random.default_rng(seed)
+        un, ln, ls, g = u.numpy(), logL.numpy(), Lstar.numpy(), group.numpy()      # views: updated in place
+        K, d = un.shape
+        self.calls += 1
+        self.max_walkers = max(self.max_walkers, K)
+        n_acc = np.zeros(chol.shape[0], dtype=np.int32)
+        for _ in range(steps):
+            z = rng.standard_normal((K, d))
+            prop = un + (np.asarray(scale)[g] * 2.38 / math.sqrt(d))[:, None] * np.einsum("kij,kj->ki", np.asarray(chol)[g], z)
+            inside = np.all((prop >= 0) & (prop <= 1), axis=1)
+            pl = np.where(inside, self._ll(np.clip(prop, 0, 1)), -np.inf)
+            ok = pl > ls
+            un[ok], ln[ok] = prop[ok], pl[ok]
+            np.add.at(n_acc, g[ok], 1)
+        return n_acc
+
+
+def test_run_device_host_side_with_a_stub_context():
+    from paper_2205_06819_b200.nested import combine_runs, run_device
+    d, sigma = 3, 0.05
+    free = [2, 5, 7]
+    theta0 = np.arange(17.0)
+    lo, hi = np.array([10.0, -1.0, 0.5]), np.array([20.0, 1.0, 2.5])
+    ctx = _StubContext([0.4, 0.6, 0.5], sigma, free, lo, hi)
+    runs = run_device(ctx, free, lo, hi, theta0, nlive=300, batch=100, mcmc_steps=25, n_runs=4, seed=7)
+    assert len(runs) == 4 and ctx.max_walkers == 400                # 4 runs x 100 walkers share every call
+    assert ctx.calls == max(r.n_iter for r in runs)                 # one device call per lock-step iteration
+    for r in runs:                                                  # a normalised Gaussian inside the cube: ln Z = 0
+        assert abs(r.logZ) < 3 * r.logZ_err + 0.06, r.logZ
+        assert abs(np.exp(r.logw).sum() - 1) < 1e-9
+    lz, err = combine_runs(runs)
+    assert abs(lz) < 4 * err + 0.05
+    mean, std = runs[0].posterior_mean_std(lambda u: lo + (hi - lo) * u)
+    want = lo + (hi - lo) * np.array([0.4, 0.6, 0.5])
+    assert np.all(np.abs(mean - want) < 5 * sigma * (hi - lo) / math.sqrt(30))
+    again = run_device(_StubContext([0.4, 0.6, 0.5], sigma, free, lo, hi), free, lo, hi, theta0, nlive=300, batch=100,
+                       mcmc_steps=25, n_runs=4, seed=7)
+    assert [r.logZ for r in again] == [r.logZ for r in runs]        # same seed, same runs
