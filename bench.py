@@ -262,20 +262,18 @@ def measure(torch, bang, idx, prec, device, flush, steps, warmup, variant=None, 
     total = D.max_over_ranks(sum(times), device="cuda" if world > 1 else None)
     name = workload_name(idx, prec) + (f"_{tag or variant}" if (tag or variant) else "")
     clocks = clk.summary()
-    unfused = bool(extra and extra.get("psf_weighting")) and not getattr(bang, "FLUX_IS_FUSED", False)
     res = {"workload": name, "B": B, "steps": steps, "ms_per_step": 1e3 * total / steps,
            "value": world * B * steps / total, "ncell": ncell, "rk": rk, "cfg": cfg, "launches": launches,
            "e2e": {"value": world * B * steps / e2e_t, "unit": UNIT, "h2d_bytes_per_step": B * W.NTHETA * 8,
                    "d2h_bytes_per_step": B * 8},
            "clocks": clocks}
-    if not unfused:
-        traffic, fma = profile_numbers(name)
-        mean_t = total / steps
-        roof = R.roofline(B * ncell, mean_t, cfg["supersample"], rk, prec, clocks.get("sm_mhz"), traffic,
-                          comps=cfg["components"], fma_pipe_pct=fma)
-        roof["kernel"] = "k_fused"
-        roof["kernel_ms_best"] = 1e3 * min(times)
-        res["roofline"] = roof
+    traffic, fma = profile_numbers(name)
+    mean_t = total / steps
+    roof = R.roofline(B * ncell, mean_t, cfg["supersample"], rk, prec, clocks.get("sm_mhz"), traffic,
+                      comps=cfg["components"], fma_pipe_pct=fma)
+    roof["kernel"] = "k_fused"
+    roof["kernel_ms_best"] = 1e3 * min(times)
+    res["roofline"] = roof
     res["ctx"] = ctx
     return res
 
@@ -359,18 +357,15 @@ def run_ours(args):
         for (i2, p2, var, extra, tag) in SWEEP:
             if (i2, p2) == (idx, prec) and var is None and extra is None:
                 continue
-            if extra and "bulge_potential" in extra and not getattr(bang, "HAS_TOTAL_POTENTIAL", False):
-                continue
             r = measure(torch, bang, i2, p2, dev, flush, max(20, min(args.steps, 50)), 3, var, extra, tag=tag)
             r.pop("ctx").close()
             r.pop("cfg")
             row = {"workload": r["workload"], "B": r["B"], "steps": r["steps"], "ms_per_step": r["ms_per_step"],
                    "evals_per_s": r["value"], "e2e": r["e2e"], "clocks": r["clocks"], "gpu_launches": r["launches"]}
-            if "roofline" in r:
-                row["roofline"] = r["roofline"]
-                row["roofline_frac"] = r["roofline"]["frac"]
-            else:
-                row["note"] = "side variant run UNFUSED through HBM scratch: no roofline is claimed for it"
+            row["roofline"] = r["roofline"]
+            row["roofline_frac"] = r["roofline"]["frac"]
+            if extra:
+                row["note"] = "widened variant (SURVEY.md sec. 8f): the census is the paper's path's, so frac understates the work done"
             sweep.append(row)
         line["sweep"] = sweep
     if rank == 0:

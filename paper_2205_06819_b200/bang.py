@@ -20,8 +20,6 @@ BULGE_HERNQUIST, BULGE_JAFFE = 0, 1
 FP32, FP64 = 0, 1
 PSF_FIELDS, PSF_FLUX = 0, 1
 POTENTIAL_SELF, POTENTIAL_TOTAL = 0, 1
-HAS_TOTAL_POTENTIAL = True        # bench.py's sweep row for reading U'
-FLUX_IS_FUSED = True              # reading G' runs inside k_fused (bench.py then reports its roofline)
 NTHETA = 17
 OK, EINVAL, ENOMEM, ECUDA, ENODATA = 0, -1, -2, -3, -4
 
