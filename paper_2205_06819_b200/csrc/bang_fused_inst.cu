@@ -56,6 +56,14 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
     p.Ftab = PolyTab<T>{static_cast<const T*>(L.Ftab), L.Ftab_first, L.Ftab_cells};
     p.quad = L.quad; p.bs_elems = (int)bs_elems<T>(L.g);
     for (int t = 0; t < NACC * S; ++t) p.W[t] = (T)L.W[t];
+    if constexpr (sizeof(T) == 4) {
+        constexpr int N = NACC * S;
+        auto w = [&](int t) { return t < N ? (float)L.W[t] : 0.f; };
+        for (int k = 0; k < (N + 1) / 2; ++k) {
+            p.W2.a[k] = make_float2(w(2 * k), w(2 * k + 1));
+            p.W2.b[k] = make_float2(w(2 * k + 1), w(2 * k + 2));
+        }
+    }
     p.theta = L.theta; p.B = L.B; p.mode = L.mode; p.nxp = L.nxp;
     p.maps = static_cast<T*>(L.maps); p.data = L.data; p.C0 = L.C0; p.logL = L.logL;
     p.slow_list = L.slow_list; p.slow_count = L.slow_count;

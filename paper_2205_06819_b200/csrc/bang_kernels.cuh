@@ -696,6 +696,49 @@ BANG_D void eval_cell(const CellK<T>& k, const T* __restrict__ bbase, const T* _
     combine_cell<T, BULGE, FLUX>(k, Bb, IbL, E1, E2, shift, vc, cosphi, oB, oV, oS, oLM);
 }
 
+// eval_cell in two halves for fp32 mode (same arithmetic, same order): cell_begin does the geometry, the table addresses
+// and ISSUES the three 128-bit table loads; cell_end consumes them.  eval_superrow calls cell_begin for the S cells of a
+// column first, so that the loads of all of them are in flight before the first polynomial is evaluated.
+struct CellF {
+    float tb, tv, r, cosphi;
+    float4 v0, v1, vv;
+};
+template <bool BULGE>
+BANG_D void cell_begin(const CellK<float>& k, const float* __restrict__ bs, const float* __restrict__ vtab, const float xp,
+                       const float yp, CellF& c) {
+    const float y2 = yp * yp;
+    const float R2 = fmaxf(fmaf(xp, xp, y2), 0x1p-32f);
+    const float r2 = fmaf(y2, k.tan2i, R2);
+    if constexpr (BULGE) {
+        const int e = max(tab_cell(R2 * k.invRb2, c.tb) - k.bfirst1, 0);
+        BANG_ASSERT(e <= k.blast);
+        const float4* p = reinterpret_cast<const float4*>(bs) + 2 * e;
+        c.v0 = p[0]; c.v1 = p[1];
+    }
+    const int cell = max(tab_cell(r2, c.tv) - k.vfirst1, 0);
+    BANG_ASSERT(cell <= k.vlast);
+    c.vv = *reinterpret_cast<const float4*>(vtab + cell * 4);
+    const float rinv = fast_rsqrt(r2);
+    c.cosphi = xp * rinv;
+    c.r = r2 * rinv;
+}
+template <bool BULGE, int SHIFT, bool FLUX>
+BANG_D void cell_end(const CellK<float>& k, const CellF& c, float& oB, float& oV, float& oS, float& oLM) {
+    float Bb = 0.f, IbL = 0.f;
+    if constexpr (BULGE) {
+        const float cs[4] = {c.v0.x, c.v0.y, c.v0.z, c.v0.w}, cj[4] = {c.v1.x, c.v1.y, c.v1.z, c.v1.w};
+        Bb = k.ampBb * horner<float, 3>(cs, c.tb);
+        IbL = k.ampIb * horner<float, 3>(cj, c.tb);
+    }
+    const float e1a = c.r * k.cexp0, e2a = c.r * k.cexp1;
+    float shift = 0.f;
+    if constexpr (!BULGE) shift = SHIFT == 1 ? e1a : (SHIFT == 2 ? e2a : fmaxf(e1a, e2a));
+    const float E1 = fast_exp2(e1a - shift), E2 = fast_exp2(e2a - shift);
+    const float cv[4] = {c.vv.x, c.vv.y, c.vv.z, c.vv.w};
+    const float vc = horner<float, 3>(cv, c.tv);
+    combine_cell<float, BULGE, FLUX>(k, Bb, IbL, E1, E2, shift, vc, c.cosphi, oB, oV, oS, oLM);
+}
+
 // The direct path: one fine cell evaluated without the per-theta table and, where s^2 leaves the scale-free tables,
 // without those either -- eq. 4-5 in closed form, eq. 6 by the N_J-node rule, eq. 10 term by term, in fp64.  Taken by the
 // rare theta whose grid spans more octaves of r^2 than the v_c table holds (|i| -> 90 deg) or whose R/R_b leaves
@@ -841,7 +884,7 @@ constexpr int lbc_nfb(int lbc, int P, int S, int NACC, int elem_bytes) {
     return (padded + 3) / 4 * 4 + 4 + row_pad(P, S, elem_bytes);
 }
 #ifndef BANG_MB_P4
-#define BANG_MB_P4 6             // resident CTAs per SM the class-0 kernels are compiled for (register budget 80 / 72)
+#define BANG_MB_P4 5             // resident CTAs per SM the class-0 kernels are compiled for (register budget 96 / 72)
 #endif
 #ifndef BANG_MB_P2
 #define BANG_MB_P2 7
@@ -856,7 +899,7 @@ constexpr int lbc_blocks(int lbc, int P, bool f64) {
 // the rotation and the store address are shared by S cells and S independent dependency chains are in flight.
 // dst[(row * 4 + observable) * NFB + x].  GUARD: some of the S rows lie past the grid (zero-weight tap padding): they
 // are written as zeros.
-template <typename T, int S, int NFB, int GRP, int PADV, bool BULGE, int SHIFT, bool GUARD, bool FLUX>
+template <typename T, int S, int NFB, int GRP, int PADV, bool BULGE, int SHIFT, bool GUARD, bool FLUX, bool SPLIT>
 BANG_D void eval_superrow(const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs, const T* __restrict__ vtab, T* __restrict__ dst,
                           const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
     const T b0 = (T)(jy0 - k.jcy);
@@ -866,6 +909,19 @@ BANG_D void eval_superrow(const CellK<T>& k, const T* __restrict__ bbase, const 
         const T px = fma(a, k.hc, bx), py = fma(-a, k.hs, by);
         T* d = dst + x + (PADV ? PADV * (x / GRP) : 0);      // row_pad: GRP is a power of two whenever PADV != 0
         BANG_ASSERT(x + (PADV ? PADV * (x / GRP) : 0) < NFB);
+        if constexpr (sizeof(T) == 4 && !GUARD && SPLIT) {     // all S cells' table loads in flight first (cell_begin)
+            CellF c[S];
+#pragma unroll
+            for (int j = 0; j < S; ++j)
+                cell_begin<BULGE>(k, bs, vtab, j == 0 ? px : fma((T)j, k.hs, px), j == 0 ? py : fma((T)j, k.hc, py), c[j]);
+#pragma unroll
+            for (int j = 0; j < S; ++j) {
+                T vB, vV, vS, vL;
+                cell_end<BULGE, SHIFT, FLUX>(k, c[j], vB, vV, vS, vL);
+                d[(j * 4 + 0) * NFB] = vB; d[(j * 4 + 1) * NFB] = vV; d[(j * 4 + 2) * NFB] = vS; d[(j * 4 + 3) * NFB] = vL;
+            }
+            continue;
+        }
 #pragma unroll
         for (int j = 0; j < S; ++j) {
             T vB, vV, vS, vL;
@@ -879,17 +935,23 @@ BANG_D void eval_superrow(const CellK<T>& k, const T* __restrict__ bbase, const 
         }
     }
 }
-template <typename T, int S, int NFB, int GRP, int PADV, bool GUARD, bool FLUX>
+template <typename T, int S, int NFB, int GRP, int PADV, bool GUARD, bool FLUX, bool SPLIT>
 BANG_D void eval_superrow_any(const unsigned comps, const CellK<T>& k, const T* __restrict__ bbase, const T* __restrict__ bs, const T* __restrict__ vtab,
                               T* __restrict__ dst, const int nfx, const int nfy, const int jy0, const int vt, const int NT) {
-    if (comps & C_BULGE) eval_superrow<T, S, NFB, GRP, PADV, true, 0, GUARD, FLUX>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+    if (comps & C_BULGE) eval_superrow<T, S, NFB, GRP, PADV, true, 0, GUARD, FLUX, SPLIT>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
     else if ((comps & (C_DISC1 | C_DISC2)) == (C_DISC1 | C_DISC2))
-        eval_superrow<T, S, NFB, GRP, PADV, false, 3, GUARD, FLUX>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else if (comps & C_DISC1) eval_superrow<T, S, NFB, GRP, PADV, false, 1, GUARD, FLUX>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
-    else eval_superrow<T, S, NFB, GRP, PADV, false, 2, GUARD, FLUX>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+        eval_superrow<T, S, NFB, GRP, PADV, false, 3, GUARD, FLUX, SPLIT>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else if (comps & C_DISC1) eval_superrow<T, S, NFB, GRP, PADV, false, 1, GUARD, FLUX, SPLIT>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
+    else eval_superrow<T, S, NFB, GRP, PADV, false, 2, GUARD, FLUX, SPLIT>(k, bbase, bs, vtab, dst, nfx, nfy, jy0, vt, NT);
 }
 
 // ---- the fused kernel ---------------------------------------------------------------------------------------------
+// fp32 mode: the composite taps as pairs for Blackwell's two-wide FMA (FFMA2): a[k] = {W[2k], W[2k+1]} serves the
+// pixels whose run starts on an even cell, b[k] = {W[2k+1], W[2k+2]} those that start on an odd one (their first tap is
+// applied on its own).  Zero beyond the taps.
+template <typename T, int N> struct TapPairs {};
+template <int N> struct TapPairs<float, N> { float2 a[(N + 1) / 2], b[(N + 1) / 2]; };
+
 template <typename T, int S, int NACC>
 struct FusedParams {
     GridC g;
@@ -898,6 +960,7 @@ struct FusedParams {
     QuadC quad;                  // reading U': the N_J-node rule for Itilde_ext
     int bs_elems;                // size of the per-theta bulge tables in shared memory, in values of T (bs_elems<T>(g))
     T W[NACC * S];               // composite x s box (*) Gaussian taps, zero padded (a4 + a5)
+    TapPairs<T, NACC * S> W2;    // the same in pairs (fp32 mode)
     const double* theta;         // [B][17]
     int B;
     int mode;                    // 0 maps, 1 likelihood (read by the MODE = 2 instantiations only)
@@ -987,6 +1050,9 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
     const T* bs = p.bs_elems ? bs_mem : nullptr;
     constexpr int nfb = lbc_nfb(LBC, P, S, NACC, (int)sizeof(T));
     constexpr int GRP = P * S, PADV = row_pad(P, S, (int)sizeof(T));
+    // the P = 4 kernels have the registers (96 in class 0) to keep the table loads of a column's S cells in flight at once;
+    // at the 72 registers of P = 2 the same ordering costs 1-2 %
+    constexpr bool SPLIT = P == 4;
     double* red = reinterpret_cast<double*>(rowbuf + (size_t)S * 4 * nfb);
 
     const GridC& g = p.g;
@@ -1043,8 +1109,8 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
             // the per-theta constants are re-read from shared memory for every super-row (a handful of broadcast loads)
             // so that they do not occupy registers during the PSF phase
             const CellK<T> k = load_cellk<T>(c);
-            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, GRP, PADV, false, FLUX>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
-            else eval_superrow_any<T, S, nfb, GRP, PADV, true, FLUX>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            if ((sr + 1) * S <= g.nfy) eval_superrow_any<T, S, nfb, GRP, PADV, false, FLUX, SPLIT>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
+            else eval_superrow_any<T, S, nfb, GRP, PADV, true, FLUX, SPLIT>(g.comps, k, bbase, bs, vtab, rowbuf, g.nfx, g.nfy, sr * S, vt, NT);
             vt = vt + 32 < NT ? vt + 32 : vt + 32 - NT;      // rotate the column ownership by one warp: the ragged last
                                                              // pass then falls on a different warp (scheduler) each time
             __syncthreads();
@@ -1068,8 +1134,25 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
 #pragma unroll
                     for (int i = 0; i < P; ++i) {
                         T xp = T(0);
+                        if constexpr (sizeof(T) == 4 && P == 4) {
+                            // FFMA2, two taps per instruction: even and odd taps accumulate in the halves of one register
+                            // pair (cells f[2m], f[2m+1] sit in an aligned pair after the vector loads), so the four
+                            // chains stay as short as the scalar ones.  Pays only where the kernel has registers to
+                            // cover the shared loads (P = 4, 96 registers: config 3 10.96 -> 10.80 ms); at P = 2 / 72
+                            // registers it changes nothing, and packing the y scatter as well spills
+                            constexpr int NTAP = NACC * S;
+                            const int base = i * S, t0 = base & 1;
+                            float2 s2 = make_float2(0.f, 0.f);
 #pragma unroll
-                        for (int t = 0; t < NACC * S; ++t) xp = fma(p.W[t], f[i * S + t], xp);
+                            for (int t = t0; t + 1 < NTAP; t += 2)
+                                s2 = __ffma2_rn(t0 ? p.W2.b[t >> 1] : p.W2.a[t >> 1], make_float2(f[base + t], f[base + t + 1]), s2);
+                            xp = s2.x + s2.y;
+                            if (t0) xp = fma(p.W[0], f[base], xp);
+                            if ((NTAP - t0) & 1) xp = fma(p.W[NTAP - 1], f[base + NTAP - 1], xp);
+                        } else {
+#pragma unroll
+                            for (int t = 0; t < NACC * S; ++t) xp = fma(p.W[t], f[i * S + t], xp);
+                        }
 #pragma unroll
                         for (int kk = 0; kk < NACC; ++kk) acc[i][kk] = fma(p.W[(NACC - 1 - kk) * S + j], xp, acc[i][kk]);
                     }
