@@ -873,7 +873,7 @@ constexpr int row_pad(int P, int S, int elem_bytes) {
 }
 // LBC: launch-bound class = the CTA-size bracket the kernel is compiled for, which fixes its register budget, the
 // row-buffer pitch (hence the shared memory per CTA) and the pitch of the data array:
-//   0: <= 128 threads, 7 (P = 2) or 6 (P = 4) CTAs per SM;  1: <= 256 threads, 3 or 2 CTAs per SM;  2: <= 512 threads
+//   0: <= 128 threads, 7 (P = 2, 72 registers) or 5 (P = 4, 96 registers) CTAs per SM;  1: <= 256 threads, 3 or 2 CTAs per SM;  2: <= 512 threads
 //   (2 CTAs per SM with P = 2, else 1).
 constexpr int lbc_threads(int lbc) { return lbc == 0 ? 128 : (lbc == 1 ? 256 : 512); }
 // plane pitch: nxp <= threads P / 4 data columns, i.e. (nxp - 1 + NACC) S cells, rounded up to a multiple of 4, plus 4
