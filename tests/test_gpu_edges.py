@@ -251,6 +251,29 @@ def test_error_codes(bang, oracle):
     assert L.bang_loglike(ctx._h, None, 3, None) == bang.EINVAL
     assert L.bang_model_maps(ctx._h, None, -1, None) == bang.EINVAL
     assert L.bang_set_data(ctx._h, None, None, None) == bang.EINVAL
+    # bang_ns_walk: argument checks, and the degenerate calls that do nothing
+    d, K = 3, 8
+    u = torch.full((K, d), 0.5, dtype=torch.float64, device="cuda")
+    ll = torch.zeros(K, dtype=torch.float64, device="cuda")
+    ls = torch.full((K,), -np.inf, dtype=torch.float64, device="cuda")
+    grp = torch.zeros(K, dtype=torch.int32, device="cuda")
+    chol, free = 0.01 * np.eye(d)[None], [2, 3, 4]
+    lo, hi = THETA[free] * 0.99, THETA[free] * 1.01
+    assert ctx.ns_walk(u, ll, ls, grp, chol, [1.0], free, lo, hi, THETA, steps=0).tolist() == [0]      # no step: no-op
+    assert torch.equal(u, torch.full_like(u, 0.5))
+    with pytest.raises(bang.BangError) as ei:
+        ctx.ns_walk(u, ll, ls, grp, chol, [1.0], [2, 3, 99], lo, hi, THETA, steps=1)                    # free index out of range
+    assert ei.value.code == bang.EINVAL
+    import ctypes as C
+    n_acc = (C.c_int * 1)()
+    fi = (C.c_int * 3)(2, 3, 4)
+    assert L.bang_ns_walk(ctx._h, K, 18, fi, lo.ctypes.data, hi.ctypes.data, THETA.ctypes.data, u.data_ptr(), ll.data_ptr(),
+                          ls.data_ptr(), grp.data_ptr(), 1, chol.ctypes.data, lo.ctypes.data, 1, 0, n_acc) == bang.EINVAL   # d > 17
+    fresh = bang.Context(cfg, precision="fp32")
+    with pytest.raises(bang.BangError) as ei:
+        fresh.ns_walk(u, ll, ls, grp, chol, [1.0], free, lo, hi, THETA, steps=1)                         # before bang_set_data
+    assert ei.value.code == bang.ENODATA
+    fresh.close()
     ctx.close()
     # a context on a stream of its own
     s = torch.cuda.Stream()

@@ -116,15 +116,18 @@ def extreme_thetas():
     return np.stack(out)
 
 
-SMALL = dict(W.config(2), nx=16, ny=12, supersample=2, jeans_nodes=32)
+SMALL_BASE = dict(W.config(2), nx=16, ny=12, supersample=2, jeans_nodes=32)
 ON_CELL_SMALL = 0.25          # s = 2, even N: fine-cell centres at ((J + 1/2)/2 - N/2) arcsec
 
 
+@pytest.mark.parametrize("variant", [{}, {"psf_weighting": 1}, {"bulge_potential": 1}, {"bulge_profile": 1}],
+                         ids=["paper", "flux_psf", "total_potential", "jaffe"])
 @pytest.mark.parametrize("prec", ["fp64", "fp32"])
-def test_radii_outside_the_tabulated_ranges_take_the_direct_path(bang, oracle, prec):
+def test_radii_outside_the_tabulated_ranges_take_the_direct_path(bang, oracle, prec, variant):
     """include/bang.h: the library's domain is the model's (R_b, R_d > 0, |i| < 90 deg, ...), not the tables': a theta
     whose grid leaves the tabulated ranges is evaluated directly (slow path), cell by cell, and must match the oracle
-    like any other."""
+    like any other -- in the paper's model and in the widened variants (readings G', U', App. B)."""
+    SMALL = dict(SMALL_BASE, **variant)
     theta = extreme_thetas()
     t0 = W.theta_true(2)
     t0[12] = 4.0
