@@ -273,6 +273,7 @@ def measure(torch, bang, idx, prec, device, flush, steps, warmup, variant=None, 
                       comps=cfg["components"], fma_pipe_pct=fma)
     roof["kernel"] = "k_fused"
     roof["kernel_ms_best"] = 1e3 * min(times)
+    roof["kernel_ms_median"] = 1e3 * statistics.median(times)
     res["roofline"] = roof
     res["ctx"] = ctx
     return res
@@ -344,7 +345,7 @@ def run_ours(args):
                            "supersample": cfg["supersample"], "sigma_pix": cfg["sigma_pix"], "r_k": m["rk"],
                            "jeans_nodes": cfg["jeans_nodes"], "fine_cells_per_theta": m["ncell"],
                            "components": comp_string(cfg["components"]), "logL_accumulation": "f64",
-                           "mask_frac": cfg.get("mask_frac", 0.0),
+                           "mask_frac": cfg.get("mask_frac", 0.0), "seed": W.SEED0 + idx,
                            "l2": "flushed between timed iterations (256 MiB rewrite)",
                            "parallelism": f"theta-sharded x{world}, every rank runs the config batch, no data-path collective"},
                 "fine_cell_evals_per_s": m["value"] * m["ncell"], "e2e": m["e2e"], "gpu_launches": m["launches"],
