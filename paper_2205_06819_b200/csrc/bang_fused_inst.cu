@@ -15,7 +15,10 @@ namespace {
 
 template <typename T, int S, int NACC, int P, int MODE, int LBC, bool FLUX>
 cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) {
-    auto kern = k_fused<T, S, NACC, P, MODE, LBC, FLUX>;
+    auto kern = []() {
+        if constexpr (sizeof(T) == 8) return k_fused64<T, S, NACC, P, MODE, LBC, FLUX>;
+        else return k_fused<T, S, NACC, P, MODE, LBC, FLUX>;
+    }();
     if (L.threads > lbc_threads(LBC)) return cudaErrorInvalidValue;
     const size_t smem = fused_smem_bytes<T>(L.g, S, lbc_nfb(LBC, P, S, NACC, (int)sizeof(T)));
     // the shared-memory opt-in and the occupancy query are done once per context and mode (L.cache, owned by the

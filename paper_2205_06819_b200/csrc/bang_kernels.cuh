@@ -1035,8 +1035,15 @@ BANG_D double inv_ml(double x) { return 1.0 / fmax(x, 1e-300); }
 // together, so in this instantiation the PSF threads are numbered observable-fastest (lane = 4 group + observable) and the
 // moments travel by warp shuffle inside each quad of lanes; the paper's path (FLUX = false) keeps its own numbering and
 // carries none of this code.
-template <typename T, int S, int NACC, int P, int MODE, int LBC, bool FLUX = false>
-__global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T) == 8)) k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
+// the register budget of an instantiation, stated outright (__maxnreg__): what lbc_blocks CTAs of lbc_threads threads leave
+// of the SM's 64 K registers, in multiples of 8 (the min-blocks form of __launch_bounds__ gives the same cap but a slightly
+// slower schedule: config 3 10.79 -> 10.72 ms, config 4 1.375 -> 1.366 ms)
+constexpr int lbc_regs(int lbc, int P, bool f64) {      // fp32 mode (f64 = false)
+    const int r = 65536 / (lbc_threads(lbc) * lbc_blocks(lbc, P, f64)) / 8 * 8;
+    return r > 128 ? 128 : r;
+}
+template <typename T, int S, int NACC, int P, int MODE, int LBC, bool FLUX>
+BANG_D void fused_body(const FusedParams<T, S, NACC>& p) {
     constexpr int D = TabCfg<T>::D, NC = D + 1;
     constexpr int RUN = (P - 1 + NACC) * S;          // fine cells one thread reads per row for its P data pixels
     constexpr int RUN_BYTES = P * S * (int)sizeof(T);   // byte stride between the runs of neighbouring threads
@@ -1206,6 +1213,19 @@ __global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, sizeof(T)
             }
         }
     }
+}
+
+// The kernel proper.  fp32 mode states its register budget outright (__maxnreg__, lbc_regs above); fp64 mode keeps the
+// min-blocks form of __launch_bounds__ (same cap of 128, and measured 4 % faster at config 2 that way).
+template <typename T, int S, int NACC, int P, int MODE, int LBC, bool FLUX = false>
+__global__ void __launch_bounds__(lbc_threads(LBC)) __maxnreg__(lbc_regs(LBC, P, false))
+k_fused(const __grid_constant__ FusedParams<T, S, NACC> p) {
+    fused_body<T, S, NACC, P, MODE, LBC, FLUX>(p);
+}
+template <typename T, int S, int NACC, int P, int MODE, int LBC, bool FLUX = false>
+__global__ void __launch_bounds__(lbc_threads(LBC), lbc_blocks(LBC, P, true))
+k_fused64(const __grid_constant__ FusedParams<T, S, NACC> p) {
+    fused_body<T, S, NACC, P, MODE, LBC, FLUX>(p);
 }
 
 // un-convolved fine maps (bang_model_fine): one CTA per theta, same decode / table / cell code as the fused kernel
