@@ -66,6 +66,7 @@ cudaError_t launch_mode(const FusedLaunch& L, FusedInfo* info, bool query_only) 
             p.W2.a[k] = make_float2(w(2 * k), w(2 * k + 1));
             p.W2.b[k] = make_float2(w(2 * k + 1), w(2 * k + 2));
         }
+        for (int t = 0; t < N; ++t) p.W2.d[t] = make_float2(w(t), w(t));
     }
     p.theta = L.theta; p.B = L.B; p.mode = L.mode; p.nxp = L.nxp;
     p.maps = static_cast<T*>(L.maps); p.data = L.data; p.C0 = L.C0; p.logL = L.logL;
