@@ -1103,7 +1103,7 @@ BANG_D void fused_body(const FusedParams<T, S, NACC>& p) {
             }
         }
 
-        constexpr bool F2Y = sizeof(T) == 4 && P == 4 && LBC == 0;    // (class 1, NACC = 10: 20 pair accumulators, measured 2 % slower)
+        constexpr bool F2Y = sizeof(T) == 4 && LBC == 0;    // (class 1, NACC = 10: 20 pair accumulators, measured 2 % slower)
         T acc[F2Y ? 1 : P][F2Y ? 1 : NACC];
         float2 acc2[F2Y ? P / 2 : 1][F2Y ? NACC : 1];      // F2Y: the running data rows of pixels (2 ip, 2 ip + 1) as pairs
         if constexpr (F2Y) {
@@ -1151,12 +1151,11 @@ BANG_D void fused_body(const FusedParams<T, S, NACC>& p) {
 #pragma unroll
                     for (int i = 0; i < P; ++i) {
                         T xp = T(0);
-                        if constexpr (sizeof(T) == 4 && P == 4) {
+                        if constexpr (sizeof(T) == 4) {
                             // FFMA2, two taps per instruction: even and odd taps accumulate in the halves of one register
                             // pair (cells f[2m], f[2m+1] sit in an aligned pair after the vector loads), so the four
-                            // chains stay as short as the scalar ones.  Pays only where the kernel has registers to
-                            // cover the shared loads (P = 4, 96 registers: config 3 10.96 -> 10.80 ms); at P = 2 / 72
-                            // registers it changes nothing, and packing the y scatter as well spills
+                            // chains stay as short as the scalar ones (config 3 10.96 -> 10.80 ms on the 96-register
+                            // kernel; on the 80-register kernel of r02b it had changed nothing)
                             constexpr int NTAP = NACC * S;
                             const int base = i * S, t0 = base & 1;
                             float2 s2 = make_float2(0.f, 0.f);
