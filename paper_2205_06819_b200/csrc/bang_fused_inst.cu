@@ -133,7 +133,9 @@ cudaError_t BANG_NAME(BANG_INST_TN, BANG_INST_S)(const FusedLaunch& L, FusedInfo
         if (L.P == 2) return launch_nacc<T, S, 2>(L, info, query_only);
     } else {
         if (L.P == 4) return launch_nacc<T, S, 4>(L, info, query_only);
+#ifdef BANG_TUNING      // fp32 mode always takes P = 4; the P = 2 kernels exist in development builds only
         if (L.P == 2) return launch_nacc<T, S, 2>(L, info, query_only);
+#endif
     }
     return cudaErrorInvalidValue;
 }

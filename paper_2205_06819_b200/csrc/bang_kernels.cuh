@@ -410,12 +410,14 @@ BANG_D float vext2(const ThetaD&, const ThetaF& df, const GridC& g, const PolyTa
     return vc2_total_f(df, g, g.comps & ~C_BULGE, Ftab, r);
 }
 template <typename R, typename T>
-BANG_D R ext_Itilde(const R s, const ThetaD& d, const ThetaF& df, const GridC& g, const PolyTab<T>& Ftab, const QuadC& q) {
+BANG_D R ext_Itilde(const R s, const ThetaD& d, const ThetaF& df, const GridC& g, const PolyTab<T>& Ftab, const QuadC& q,
+                    const int k0 = 0, const int kstep = 1) {
+    // (k0, kstep): the nodes k0, k0 + kstep, ... only -- the table build deals one rule out over four lanes
     const R L = sqrt(fma(s, s, R(1)));
     const R Rb = (R)d.Rb;
     R sum = R(0);
 #pragma unroll 1
-    for (int k = 0; k < q.NJ; ++k) {
+    for (int k = k0; k < q.NJ; k += kstep) {
         R a, b;
         quad_node(q, k, a, b);
         const R dd = L * a;                               // x~ - s
@@ -460,17 +462,27 @@ BANG_D void build_bulge_tables(const ThetaC<T>& c, const GridC& g, const FitC& f
     {
         const ThetaF df{(float)c.d.GMb, (float)c.d.Rb, {(float)c.d.Ad[0], (float)c.d.Ad[1]},
                         {(float)c.d.inv2Rd[0], (float)c.d.inv2Rd[1]}, (float)c.d.Ah, (float)c.d.hs};
-        for (int i = threadIdx.x; i <= ncoarse; i += blockDim.x) {
-            double s2;
-            if (i == ncoarse) s2 = c.d.s2near;
-            else {
-                const int pn = i / q.ND, k = i - pn * q.ND;
-                s2 = exp2((double)(e0 + pn * q.span) + 0.5 * q.span * (q.bx[k] + 1.0));
+        // every evaluation of the rule is dealt out over four neighbouring lanes (nodes k = part, part + 4, ...; the partial
+        // sums meet by shuffle), so that the ~70 evaluations of a theta keep a 64-thread CTA busy as well as a 128-thread one
+        for (int base = 0; base < 4 * (ncoarse + 1); base += blockDim.x) {
+            const int item = base + threadIdx.x, i = item >> 2, part = item & 3;
+            const bool on = i <= ncoarse;
+            double s2 = 1.0;
+            if (on) {
+                if (i == ncoarse) s2 = c.d.s2near;
+                else {
+                    const int pn = i / q.ND, k = i - pn * q.ND;
+                    s2 = exp2((double)(e0 + pn * q.span) + 0.5 * q.span * (q.bx[k] + 1.0));
+                }
             }
-            T v;
-            if constexpr (sizeof(T) == 4) v = ext_Itilde<float, float>(sqrtf((float)s2), c.d, df, g, Ftab, q);
-            else v = (T)ext_Itilde<double, T>(sqrt(s2), c.d, df, g, Ftab, q);
-            coarse[i] = i == ncoarse ? v : (T)log(fmax((double)v, 1e-300));
+            T v = T(0);
+            if (on) {
+                if constexpr (sizeof(T) == 4) v = ext_Itilde<float, float>(sqrtf((float)s2), c.d, df, g, Ftab, q, part, 4);
+                else v = (T)ext_Itilde<double, T>(sqrt(s2), c.d, df, g, Ftab, q, part, 4);
+            }
+            v += __shfl_xor_sync(0xffffffffu, v, 1);
+            v += __shfl_xor_sync(0xffffffffu, v, 2);
+            if (on && part == 0) coarse[i] = i == ncoarse ? v : (T)log(fmax((double)v, 1e-300));
         }
     }
     __syncthreads();
