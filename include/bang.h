@@ -141,6 +141,19 @@ int bang_model_fine(bang_ctx *ctx, const double *theta_dev, int B, void *fine_de
  * Asynchronous. */
 int bang_loglike(bang_ctx *ctx, const double *theta_dev, int B, double *logL_dev);
 
+/* bang_loglike for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): same arguments, same kernels, same results, but NO allocation on its path -- no cudaMalloc, cudaFree or
+ * allocating library routine.  bang_loglike keeps the list through which the fused kernel hands theta outside its tabulated
+ * ranges to the direct-path kernel in a buffer that grows with B; here that list lives in a file-scope static __device__
+ * array of BANG_NOALLOC_MAX_B entries (256 KiB + 256 B, held by every GPU that loads the library until the process exits;
+ * its device address is taken with cudaGetSymbolAddress at bang_create, once per device).  B > BANG_NOALLOC_MAX_B returns
+ * BANG_EINVAL with a message in bang_last_error (split the batch, or call bang_loglike).  theta_dev, logL_dev: DEVICE, as
+ * for bang_loglike; asynchronous on the context's stream.  The array is ONE per device, shared by every call and every
+ * context, and keeps the last call's contents (the call clears the counters it needs at zero): calls that overlap on the
+ * GPU -- two streams, two contexts on one device -- race on it; calls ordered on one stream do not. */
+#define BANG_NOALLOC_MAX_B 65536
+int bang_loglike_noalloc(bang_ctx *ctx, const double *theta_dev, int B, double *logL_dev);
+
 /* The replacement step of nested sampling on the device (the worst live point is
  * replaced by one of higher likelihood found by MCMC): K constrained random walks of `steps` Metropolis steps in lock-step,
  * each step = proposal kernel -> bang_loglike on the K proposals -> accept kernel, with walkers, proposals and their

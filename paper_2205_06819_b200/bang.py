@@ -21,10 +21,11 @@ FP32, FP64 = 0, 1
 PSF_FIELDS, PSF_FLUX = 0, 1
 POTENTIAL_SELF, POTENTIAL_TOTAL = 0, 1
 NTHETA = 17
+NOALLOC_MAX_B = 65536            # include/bang.h: BANG_NOALLOC_MAX_B
 OK, EINVAL, ENOMEM, ECUDA, ENODATA = 0, -1, -2, -3, -4
 
 EXPORTS = ["bang_create", "bang_set_data", "bang_model_maps", "bang_model_fine", "bang_loglike", "bang_loglike_host",
-           "bang_model_maps_host", "bang_ns_walk", "bang_get_geometry", "bang_launch_count", "bang_probe_peaks", "bang_ml_from_colour", "bang_destroy", "bang_strerror",
+           "bang_model_maps_host", "bang_loglike_noalloc", "bang_ns_walk", "bang_get_geometry", "bang_launch_count", "bang_probe_peaks", "bang_ml_from_colour", "bang_destroy", "bang_strerror",
            "bang_last_error"]
 
 
@@ -64,7 +65,8 @@ def lib():
         L.bang_create.restype = ip
         L.bang_set_data.argtypes = [vp, vp, vp, vp]
         L.bang_set_data.restype = ip
-        for name in ("bang_model_maps", "bang_model_fine", "bang_loglike", "bang_loglike_host", "bang_model_maps_host"):
+        for name in ("bang_model_maps", "bang_model_fine", "bang_loglike", "bang_loglike_noalloc", "bang_loglike_host",
+                     "bang_model_maps_host"):
             f = getattr(L, name)
             f.argtypes, f.restype = [vp, vp, ip, vp], ip
         L.bang_get_geometry.argtypes = [vp, C.POINTER(ip), C.POINTER(ip), C.POINTER(ip)]
@@ -190,6 +192,18 @@ class Context:
             if out is None:
                 out = torch.empty((B,), dtype=torch.float64, device=self.device)
             self._check(lib().bang_loglike(self._h, t.data_ptr(), B, out.data_ptr()))
+        return out
+
+    def loglike_noalloc(self, theta, out):
+        """bang_loglike_noalloc: theta [B][17] float64 device tensor, out [B] float64 device tensor, both made by the
+        caller (this wrapper allocates nothing either); B <= NOALLOC_MAX_B.  Asynchronous on the context's stream."""
+        torch = self._torch
+        assert torch.is_tensor(theta) and theta.dtype == torch.float64 and theta.is_contiguous() and theta.device == self.device
+        assert torch.is_tensor(out) and out.dtype == torch.float64 and out.is_contiguous() and out.device == self.device
+        B = theta.shape[0]
+        assert theta.shape == (B, NTHETA) and out.shape == (B,)
+        with self._on_stream():
+            self._check(lib().bang_loglike_noalloc(self._h, theta.data_ptr(), B, out.data_ptr()))
         return out
 
     def loglike_host(self, theta: np.ndarray, out: np.ndarray | None = None) -> np.ndarray:

@@ -41,6 +41,7 @@ struct bang_ctx {
     // direct path (bang_slow.cuh): list of the theta k_fused leaves to k_slow, {count, CTAs done}, capacity; 0 = the grid
     // is too large for k_slow's shared memory (such theta are then reported as out of domain)
     int* slow_list = nullptr; int* slow_cnt = nullptr; int slow_cap = 0; size_t slow_smem = 0;
+    int* na_scratch = nullptr;             // device address of g_noalloc_scratch on this context's device (bang_loglike_noalloc)
     double* W_dev = nullptr;               // composite taps on the device (direct path)
     bool fine_ready = false;               // k_fine's shared-memory opt-in done (once per context)
     // bang_ns_walk scratch: proposals [K][d], their theta [K][17] and likelihoods [K], Cholesky factors + scales, counts
@@ -49,7 +50,36 @@ struct bang_ctx {
     char err[512] = {0};
 };
 
+// ---- scratch of the allocation-free entry point (bang_loglike_noalloc) ---------------------------------------------------
+// The fused kernel hands the theta whose radii leave its tables to the direct-path kernel through a list in device memory
+// (bang_slow.cuh); bang_loglike keeps that list in a cudaMalloc'ed buffer that grows with B.  Callers that must not
+// allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc) get the same two kernels with the list in
+// this file-scope array instead: [0] = number of entries, [1] = CTAs of k_slow that have finished, [64 ..] = the entries.
+// 256 KiB + 256 B, held by every GPU that loads the library until the process exits.  ONE array per device, shared by every
+// call and every context: calls that overlap on the GPU (two streams) race on it.
+#define BANG_NOALLOC_MAX_B_IMPL 65536
+static __device__ __align__(256) int g_noalloc_scratch[64 + BANG_NOALLOC_MAX_B_IMPL];
+static_assert(BANG_NOALLOC_MAX_B_IMPL == BANG_NOALLOC_MAX_B, "include/bang.h states the limit");
+// In host code `g_noalloc_scratch` is a host-side stand-in for the symbol, NOT a device address: the address a kernel may be
+// given comes from cudaGetSymbolAddress, asked once per device with that device current (bang_create).
+constexpr int kMaxDevices = 64;
+static int* g_noalloc_ptr[kMaxDevices] = {nullptr};
+
 namespace {
+
+// device address of the scratch array on the CURRENT device (which must be `device`); NULL + the CUDA error on failure
+cudaError_t noalloc_scratch_address(int device, int** out) {
+    *out = nullptr;
+    if (device < 0 || device >= kMaxDevices) return cudaErrorInvalidDevice;
+    if (!g_noalloc_ptr[device]) {
+        int* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        g_noalloc_ptr[device] = ptr;
+    }
+    *out = g_noalloc_ptr[device];
+    return cudaSuccess;
+}
 
 int fail(bang_ctx* c, int code, const char* fmt, ...) {
     if (c) {
@@ -364,6 +394,27 @@ int run_slow(bang_ctx* ctx, const double* theta_dev, int mode, void* maps_dev, d
     CU(cudaGetLastError());
     return BANG_OK;
 }
+// bang_loglike with no allocation anywhere on its path: the same k_fused + k_slow launches, the direct-path list in the
+// file-scope array above.  No cudaMalloc / cudaFree / allocating routine is called here or below (make_launch, the launchers
+// and fail() use fixed storage; the first call per context does the kernel's shared-memory opt-in and occupancy query).
+template <typename T>
+int run_slow_noalloc(bang_ctx* ctx, const double* theta_dev, double* logL_dev) {
+    if (!ctx->slow_smem) return BANG_OK;
+    SlowParams<T> p{};
+    p.g = ctx->g;
+    p.btab = PolyTab<T>{static_cast<const T*>(ctx->btab), ctx->btab_first, ctx->btab_cells};
+    p.Ftab = PolyTab<T>{static_cast<const T*>(ctx->Ftab), ctx->Ftab_first, ctx->Ftab_cells};
+    p.direct = make_direct(ctx);
+    p.W = ctx->W_dev; p.nacc = ctx->nacc;
+    p.theta = theta_dev; p.slow_list = ctx->na_scratch + 64; p.slow_count = ctx->na_scratch; p.done = ctx->na_scratch + 1;
+    p.maps = nullptr; p.data = ctx->data; p.P = ctx->P; p.gmax = data_gmax(ctx);
+    p.C0 = ctx->C0; p.logL = logL_dev;
+    k_slow<T, 1><<<ctx->n_sm, 256, ctx->slow_smem, ctx->stream>>>(p);
+    ctx->launches += 1;
+    CU(cudaGetLastError());
+    return BANG_OK;
+}
+
 template <typename T>
 int setup_slow(bang_ctx* ctx) {
     const size_t smem = slow_smem_bytes<T>(ctx->g, ctx->nacc);
@@ -616,6 +667,8 @@ int bang_create(bang_ctx** out, const bang_grid* grid, const bang_psf* psf, cons
             cudaStreamSynchronize(ctx->stream) != cudaSuccess) { rc = BANG_ECUDA; break; }
         rc = f64 ? setup_slow<double>(ctx) : setup_slow<float>(ctx);
         if (rc != BANG_OK) break;
+        // the allocation-free entry point's scratch: its device address on THIS device (current here: DeviceGuard above)
+        if (noalloc_scratch_address(device, &ctx->na_scratch) != cudaSuccess) { rc = BANG_ECUDA; break; }
         // does the fused kernel fit (shared memory, registers)?
         FusedLaunch L = make_launch(ctx, nullptr, 1, 0, nullptr, nullptr);
         FusedInfo info{};
@@ -682,6 +735,28 @@ int bang_loglike(bang_ctx* ctx, const double* theta_dev, int B, double* logL_dev
     ctx->launches += 1;
     return ctx->model.precision == BANG_FP64 ? run_slow<double>(ctx, theta_dev, 1, nullptr, logL_dev)
                                              : run_slow<float>(ctx, theta_dev, 1, nullptr, logL_dev);
+}
+
+int bang_loglike_noalloc(bang_ctx* ctx, const double* theta_dev, int B, double* logL_dev) {
+    if (!ctx) return BANG_EINVAL;
+    if (B < 0 || (B > 0 && (!theta_dev || !logL_dev))) return fail(ctx, BANG_EINVAL, "bang_loglike_noalloc: bad arguments");
+    if (B > BANG_NOALLOC_MAX_B)
+        return fail(ctx, BANG_EINVAL, "bang_loglike_noalloc: B = %d exceeds BANG_NOALLOC_MAX_B = %d (the static scratch holds one "
+                                      "list entry per theta); split the batch or call bang_loglike", B, BANG_NOALLOC_MAX_B);
+    if (!ctx->has_data) return fail(ctx, BANG_ENODATA, "bang_loglike_noalloc: no data loaded");
+    if (!ctx->na_scratch) return fail(ctx, BANG_ECUDA, "bang_loglike_noalloc: the scratch symbol has no address on device %d", ctx->device);
+    if (B == 0) return BANG_OK;
+    ON_DEVICE(ctx);
+    // the array keeps the last call's contents: the two counters must start at zero (k_slow resets them when it finishes,
+    // but a call that failed half-way, or another context's, may not have)
+    CU(cudaMemsetAsync(ctx->na_scratch, 0, 64 * sizeof(int), ctx->stream));
+    FusedLaunch L = make_launch(ctx, theta_dev, B, 1, nullptr, logL_dev);
+    L.slow_list = ctx->slow_smem ? ctx->na_scratch + 64 : nullptr;
+    L.slow_count = ctx->na_scratch;
+    CU(dispatch_fused(ctx, L, nullptr, false));
+    ctx->launches += 1;
+    return ctx->model.precision == BANG_FP64 ? run_slow_noalloc<double>(ctx, theta_dev, logL_dev)
+                                             : run_slow_noalloc<float>(ctx, theta_dev, logL_dev);
 }
 
 int bang_ns_walk(bang_ctx* ctx, int K, int d, const int* free_idx_host, const double* lo_host, const double* hi_host,
